@@ -1,0 +1,175 @@
+/*
+ * fpcl.h -- C ABI of the B200-native cubic Fokker-Planck closure hot path (arxiv/paper_2606_15622).
+ *
+ * One library (libfpcl.so, hand-written CUDA for sm_100a) exposes the per-cell, per-time-step closure path of
+ * the paper's particle cubic-FP solver: PAPER.md Algorithm 1 (:205-225, physics closure) and Algorithm 2
+ * (:250-270, surrogate closure).  Every step of the path runs in this library's kernels; callers only own memory.
+ *
+ * Conventions
+ *  - C99 ABI, no exceptions.  Every call returns FP_OK (0) or a negative FP_ERR_* code; fp_last_error(ctx)
+ *    gives a human-readable string for the last failure on that context.
+ *  - Pointers are DEVICE pointers unless the name starts with h_ (host).  The caller owns every particle, grid,
+ *    coefficient and weight buffer; the library never allocates or frees them.  The library owns only fp_ctx and
+ *    the scratch sized at fp_create (sort ping-pong buffers, digit histograms, uploaded MLP parameters).
+ *  - All calls are asynchronous on the caller's stream (a cudaStream_t passed as void*; NULL = legacy default
+ *    stream) and never synchronise the host.
+ *  - Numerical trouble in a cell is NOT an error code: it sets FP_FLAG_* bits in flags[cell] and the cell gets the
+ *    documented fallback (readings R3-c, R5).
+ *  - Particle arrays are SoA fp32: x, y, vx, vy, vz [np] and a persistent particle id pid [np] (uint32) that
+ *    travels with the particle through the sort and seeds its random stream (R6).
+ *  - Moment record per cell, fp64, row-major (R0):
+ *      FULL (29): N, U1..3, P11,P12,P13,P22,P23,P33, t111,t112,t113,t122,t123,t133,t222,t223,t233,t333,
+ *                 F11,F12,F13,F22,F23,F33 (F_ij = <c^2 c_i c_j>), g1,g2,g3 (g_i = <c^4 c_i>)
+ *      LITE (13): N, U1..3, P(6), h1,h2,h3 (h_i = <c^2 c_i>)
+ *    with c = v - U and <.> the plain 1/N mean over the cell's particles.
+ *  - Coefficient record per cell (9, fp32): c11,c12,c13,c22,c23,c33,gamma1,gamma2,gamma3.
+ */
+#ifndef FPCL_H
+#define FPCL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* error codes */
+#define FP_OK               0
+#define FP_ERR_ARG         (-1)   /* null / misaligned pointer, size mismatch, bad enum                  */
+#define FP_ERR_STATE       (-2)   /* call sequence violated (e.g. np > max_particles)                     */
+#define FP_ERR_CUDA        (-3)   /* a CUDA runtime call failed; see fp_last_error                        */
+#define FP_ERR_UNSUPPORTED (-4)   /* e.g. an MLP wider than the fused kernel supports                     */
+
+/* per-cell flag bits written to flags[cell] */
+#define FP_FLAG_EMPTY      1u     /* N == 0: outputs zero                                                 */
+#define FP_FLAG_LOWCOUNT   2u     /* N < min_count: Langevin coefficients c = -delta/tau, gamma = 0        */
+#define FP_FLAG_SINGULAR   4u     /* theta <= 0, |pivot| < 1e-14 or non-finite solution: Langevin          */
+#define FP_FLAG_ILLCOND    8u     /* scaled system ill-conditioned (estimate), solution kept               */
+#define FP_FLAG_ALPHA     16u     /* alpha^2 (Eq. 15) non-finite or < 1e-6: alpha := 1                      */
+#define FP_FLAG_SKIPPED   32u     /* velocity update skipped: N < 2 or theta <= 0                           */
+#define FP_FLAG_NONFINITE 64u     /* surrogate produced a non-finite value: Langevin                        */
+
+/* wall kinds */
+#define FP_WALL_NONE     0
+#define FP_WALL_DIFFUSE  1        /* diffuse isothermal re-emission                          */
+#define FP_WALL_PERIODIC 2
+
+typedef struct fp_ctx fp_ctx;
+
+typedef struct {
+    int32_t kind;                 /* FP_WALL_*                                                             */
+    float   theta_w;              /* wall temperature as k T_w / m                                          */
+    float   ux, uy, uz;           /* wall velocity                                                          */
+} fp_wall;
+
+/* POD, host memory, copied at fp_create. */
+typedef struct {
+    int32_t  nx, ny;              /* uniform Cartesian grid; ny = 1 for the 1D Couette case                */
+    float    x0, y0, dx, dy;      /* domain origin and cell size (cell index: DESIGN.md R1)                */
+    int64_t  max_particles;       /* scratch is sized for this                                              */
+    float    dt;                  /* time step                                                              */
+    float    tau;                 /* global relaxation time; ignored where a per-cell tau array is given    */
+    float    eps2_scale;          /* multiplies the default eps^2 (R2-e); 0 disables the cubic term         */
+    int32_t  min_count;           /* exact closure: cells with N < min_count use Langevin (R3-c)            */
+    int32_t  min_count_mlp;       /* surrogate closure: same, usually 2                                     */
+    int32_t  conserve_mode;       /* 0 = Eq. 13/15 only; 1 = + exact recentre/rescale per cell (R5.5)       */
+    uint64_t seed;                /* Philox key                                                             */
+    fp_wall  wall[4];             /* xmin, xmax, ymin, ymax                                                 */
+    int32_t  body_kind;           /* 0 none, 1 embedded diffuse cylinder                                    */
+    float    body_cx, body_cy, body_R, body_theta_w;
+} fp_params;
+
+/* MLP surrogate description.  h_dims is a host array of n_layers+1 widths;
+ * W[l] / b[l] are host arrays of DEVICE pointers to fp32 weights, row-major [out][in], and biases.
+ * x_mean/x_scale [n_in], y_mean/y_scale [9] are DEVICE pointers.  act 0 = SiLU, 1 = ReLU (hidden layers only;
+ * the head is linear).  feature_set 0 = 13 inputs (n, U1..3, T, pi11,pi12,pi13,pi22,pi23, q1..3), 1 = the paper's
+ * 16 inputs (R4).  n = N * n_scale, T = theta / theta_ref. */
+typedef struct {
+    int32_t             n_layers;
+    const int32_t*      h_dims;
+    const float* const* W;
+    const float* const* b;
+    const float*        x_mean;
+    const float*        x_scale;
+    const float*        y_mean;
+    const float*        y_scale;
+    int32_t             act;
+    int32_t             feature_set;
+    float               n_scale;
+    float               theta_ref;
+} fp_mlp;
+
+/* Create / destroy a context on the current CUDA device.  fp_create validates h_params (nx, ny >= 1,
+ * dx, dy > 0, max_particles >= 0, nx*ny < 2^27) and allocates scratch; fp_destroy frees it. */
+int fp_create(fp_ctx** out, const fp_params* h_params);
+int fp_destroy(fp_ctx* ctx);
+const char* fp_last_error(const fp_ctx* ctx);
+/* Library version / build string (static storage). */
+const char* fp_version(void);
+
+/* a2 -- cell index + stable sort (R1).  key = iy*nx + ix with
+ * ix = clamp(floorf((x - x0) * (1/dx)), 0, nx-1) in fp32.  Writes the permuted SoA into the *_out arrays (which
+ * may not alias the inputs), cell_start[ncell+1] (cell_start[k] = #particles with key < k) and, if non-null,
+ * perm[np] with perm[k] = input index of the particle now at position k.  Equal keys keep input order. */
+int fp_sort_by_cell(fp_ctx* ctx, int64_t np,
+                    const float* x, const float* y, const float* vx, const float* vy, const float* vz,
+                    const uint32_t* pid,
+                    float* x_out, float* y_out, float* vx_out, float* vy_out, float* vz_out, uint32_t* pid_out,
+                    int32_t* cell_start, uint32_t* perm /* nullable */, void* stream);
+
+/* a3 -- segmented gather of the velocity moments over cell-sorted particles.
+ * mode 0 = LITE (13 doubles/cell), 1 = FULL (29 doubles/cell).  mom is [ncell * stride] fp64. */
+int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
+                    const int32_t* cell_start, int32_t mode, double* mom, void* stream);
+
+/* a4 -- exact cubic-FP closure: assemble and solve the 9x9 moment-matching system per cell (Eq. 10
+ * :121, Table 1 :130-136; derivation DESIGN.md R2, scaling and flags R3).  tau_cell nullable (then params.tau).
+ * coef [ncell*9] fp32, flags [ncell] (overwritten).  kappa_est nullable: if given receives the
+ * library's estimate (a lower bound) of the condition number of the scaled system, the same number that
+ * decides FP_FLAG_ILLCOND (>= 1e8): max(||A||_inf ||y||_inf / ||b||_inf, max|pivot| / min|pivot|). */
+int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell /* nullable */,
+                     float* coef, uint32_t* flags, double* kappa_est /* nullable */, void* stream);
+
+/* a5 -- fused MLP surrogate: features -> standardise -> dense layers -> de-standardise (PAPER.md:264, :309,
+ * :327).  mom_stride 13 or 29.  relax_w in (0,1]: coef <- w*new + (1-w)*old; 1 overwrites.
+ * Parameters are uploaded to context scratch when h_mlp's pointers/shape change (cached between calls). */
+int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell /* nullable */,
+                   const fp_mlp* h_mlp, float relax_w, float* coef, uint32_t* flags, void* stream);
+
+/* a6 -- FP velocity update, in place on cell-sorted vx, vy, vz (Eq. 13-15 :150-181; R5, R6).
+ * step is the Philox counter word for time.  flags [ncell] are OR-ed with FP_FLAG_ALPHA / FP_FLAG_SKIPPED. */
+int fp_velocity_update(fp_ctx* ctx, int64_t np, float* vx, float* vy, float* vz, const uint32_t* pid,
+                       const int32_t* cell_start, const double* mom, int32_t mom_stride, const float* coef,
+                       const float* tau_cell /* nullable */, uint64_t step, uint32_t* flags, void* stream);
+
+/* a0 + a1 -- streaming (Eq. 16 :187) and diffuse isothermal walls (:214, :674; R7),
+ * in place. */
+int fp_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
+                    const uint32_t* pid, uint64_t step, void* stream);
+
+/* a7 -- one whole step in the order of Algorithm 1/2: stream -> walls -> sort -> moments -> closure -> update.
+ * State is read from (and streamed in place in) the *_a arrays and the cell-sorted, updated state is written to
+ * the *_b arrays; the caller swaps a and b between steps.  closure 0 = exact (mom must hold ncell*29 doubles),
+ * 1 = surrogate (ncell*13 doubles, LITE gather).  tau_mode 0: params.tau everywhere; 1: per-cell
+ * tau = tau_ref_n / N computed on the device from the counts and written to tau_cell [ncell] (must be non-null;
+ * PAPER.md:83 tau = 2 mu / p ~ 1/n).  relax_w as in fp_closure_mlp. */
+int fp_step(fp_ctx* ctx, int64_t np,
+            float* x_a, float* y_a, float* vx_a, float* vy_a, float* vz_a, uint32_t* pid_a,
+            float* x_b, float* y_b, float* vx_b, float* vy_b, float* vz_b, uint32_t* pid_b,
+            int32_t closure, const fp_mlp* h_mlp, float relax_w,
+            int32_t tau_mode, float tau_ref_n, float* tau_cell /* nullable unless tau_mode 1 */,
+            uint64_t step, double* mom, float* coef, uint32_t* flags, int32_t* cell_start, void* stream);
+
+/* Host-buffer convenience used by the end-to-end measurement: uploads the six SoA arrays from host memory
+ * (pinned or pageable), runs fp_step on internally held device buffers sized max_particles, and downloads the
+ * updated SoA plus cell_start, flags and coef back into the host arrays.  Synchronises the stream before
+ * returning.  h_* are HOST pointers; h_coef [ncell*9], h_flags [ncell], h_cell_start [ncell+1]. */
+int fp_step_host(fp_ctx* ctx, int64_t np,
+                 float* h_x, float* h_y, float* h_vx, float* h_vy, float* h_vz, uint32_t* h_pid,
+                 int32_t closure, const fp_mlp* h_mlp, float relax_w, uint64_t step,
+                 float* h_coef, uint32_t* h_flags, int32_t* h_cell_start, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FPCL_H */

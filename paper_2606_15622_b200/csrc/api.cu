@@ -1,0 +1,175 @@
+// api.cu -- context life cycle and the composition of one step (Algorithm 1 :205-225 and Algorithm 2
+// :250-270): stream -> walls -> sort -> moments -> closure -> update, all on one stream with no host
+// synchronisation and no allocation inside (scratch lives in fp_ctx).
+#include <math.h>
+#include <new>
+
+#include "common.cuh"
+
+static const char* k_version = "fpcl 0.1 (sm_100a)";
+
+extern "C" const char* fp_version(void) { return k_version; }
+
+extern "C" const char* fp_last_error(const fp_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+static void fp_free_all(fp_ctx* c)
+{
+    cudaFree(c->key_a); cudaFree(c->key_b); cudaFree(c->idx_a); cudaFree(c->idx_b);
+    cudaFree(c->block_hist); cudaFree(c->bin_total);
+    for (int s = 0; s < 2; ++s) { for (int k = 0; k < 5; ++k) cudaFree(c->hs_f[s][k]); cudaFree(c->hs_pid[s]); }
+    cudaFree(c->hs_mom); cudaFree(c->hs_coef); cudaFree(c->hs_flags); cudaFree(c->hs_cell_start);
+    cudaFree(c->mlp.blob);
+}
+
+extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
+{
+    if (!out || !h_params) return FP_ERR_ARG;
+    *out = nullptr;
+    const fp_params& q = *h_params;
+    if (q.nx < 1 || q.ny < 1 || !(q.dx > 0.f) || !(q.dy > 0.f) || q.max_particles < 0 ||
+        (int64_t)q.nx * q.ny >= ((int64_t)1 << 27) || q.max_particles >= ((int64_t)1 << 31) ||
+        !(q.tau > 0.f) || (q.conserve_mode != 0 && q.conserve_mode != 1))
+        return FP_ERR_ARG;
+    for (int k = 0; k < 4; ++k) if (q.wall[k].kind < 0 || q.wall[k].kind > 2) return FP_ERR_ARG;
+    fp_ctx* c = new (std::nothrow) fp_ctx();
+    if (!c) return FP_ERR_STATE;
+    c->err[0] = 0;
+    c->p = q;
+    c->ncell = q.nx * q.ny;
+    int bits = 0;
+    while (((int64_t)1 << bits) < (int64_t)c->ncell) ++bits;
+    c->key_bits = bits;
+    // fp32, each operation rounded separately (R1, R7)
+    volatile float inv_dx = 1.0f / q.dx, inv_dy = 1.0f / q.dy;
+    volatile float wx = (float)q.nx * q.dx, wy = (float)q.ny * q.dy;
+    volatile float xmax = q.x0 + wx, ymax = q.y0 + wy;
+    c->inv_dx = inv_dx; c->inv_dy = inv_dy;
+    c->xmin = q.x0; c->ymin = q.y0; c->xmax = xmax; c->ymax = ymax;
+    c->xmax_in = nextafterf(xmax, -INFINITY); c->ymax_in = nextafterf(ymax, -INFINITY);
+    volatile float Lx = xmax - q.x0, Ly = ymax - q.y0;
+    c->Lx = Lx; c->Ly = Ly;
+    if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return FP_ERR_CUDA; }
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && sms > 0) c->num_sms = sms;
+    const size_t n = (size_t)(q.max_particles > 0 ? q.max_particles : 1);
+    const size_t nblocks = (n + 2047) / 2048;
+    c->block_hist_elems = 512 * nblocks;
+    bool ok = cudaMalloc((void**)&c->key_a, n * 4) == cudaSuccess && cudaMalloc((void**)&c->key_b, n * 4) == cudaSuccess &&
+              cudaMalloc((void**)&c->idx_a, n * 4) == cudaSuccess && cudaMalloc((void**)&c->idx_b, n * 4) == cudaSuccess &&
+              cudaMalloc((void**)&c->block_hist, c->block_hist_elems * 4) == cudaSuccess &&
+              cudaMalloc((void**)&c->bin_total, 512 * 4) == cudaSuccess;
+    if (!ok) { fp_free_all(c); delete c; cudaGetLastError(); return FP_ERR_CUDA; }
+    *out = c;
+    return FP_OK;
+}
+
+extern "C" int fp_destroy(fp_ctx* ctx)
+{
+    if (!ctx) return FP_ERR_ARG;
+    cudaDeviceSynchronize();
+    fp_free_all(ctx);
+    delete ctx;
+    return FP_OK;
+}
+
+// per-cell tau = tau_ref_n / N (tau = 2 mu / p ~ 1/n for Maxwell molecules); N = 0 -> params.tau
+__global__ void tau_kernel(const int32_t* __restrict__ cell_start, int32_t ncell, float tau_ref_n, float tau_default,
+                           float* __restrict__ tau_cell)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < ncell) {
+        const int32_t n = cell_start[i + 1] - cell_start[i];
+        tau_cell[i] = n > 0 ? tau_ref_n / (float)n : tau_default;
+    }
+}
+
+int fpi_tau_from_counts(fp_ctx* ctx, const int32_t* cell_start, float tau_ref_n, float* tau_cell, cudaStream_t st)
+{
+    tau_kernel<<<fp_div_up(ctx->ncell, 256), 256, 0, st>>>(cell_start, ctx->ncell, tau_ref_n, ctx->p.tau, tau_cell);
+    FP_LAUNCH_OK(ctx);
+    return FP_OK;
+}
+
+extern "C" int fp_step(fp_ctx* ctx, int64_t np,
+                       float* x_a, float* y_a, float* vx_a, float* vy_a, float* vz_a, uint32_t* pid_a,
+                       float* x_b, float* y_b, float* vx_b, float* vy_b, float* vz_b, uint32_t* pid_b,
+                       int32_t closure, const fp_mlp* h_mlp, float relax_w,
+                       int32_t tau_mode, float tau_ref_n, float* tau_cell,
+                       uint64_t step, double* mom, float* coef, uint32_t* flags, int32_t* cell_start, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    if (np < 0 || !mom || !coef || !flags || !cell_start || (closure != 0 && closure != 1) || (tau_mode != 0 && tau_mode != 1))
+        return fp_fail(ctx, FP_ERR_ARG, "fp_step: bad argument");
+    if (closure == 1 && !h_mlp) return fp_fail(ctx, FP_ERR_ARG, "fp_step: surrogate closure needs h_mlp");
+    if (tau_mode == 1 && !tau_cell) return fp_fail(ctx, FP_ERR_ARG, "fp_step: tau_mode 1 needs tau_cell");
+    if (np > ctx->p.max_particles) return fp_fail(ctx, FP_ERR_STATE, "fp_step: np > max_particles");
+    if (np > 0 && (!x_a || !y_a || !vx_a || !vy_a || !vz_a || !pid_a || !x_b || !y_b || !vx_b || !vy_b || !vz_b || !pid_b))
+        return fp_fail(ctx, FP_ERR_ARG, "fp_step: null particle pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    // a0 + a1 (+ cell keys of the streamed positions)
+    if ((rc = fpi_stream_walls(ctx, np, x_a, y_a, vx_a, vy_a, vz_a, pid_a, step, ctx->key_b, st)) != FP_OK) return rc;
+    // a2
+    if ((rc = fpi_sort_with_keys(ctx, np, ctx->key_b, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b,
+                                 cell_start, nullptr, st)) != FP_OK) return rc;
+    const float* tau_use = nullptr;
+    if (tau_mode == 1) {
+        if ((rc = fpi_tau_from_counts(ctx, cell_start, tau_ref_n, tau_cell, st)) != FP_OK) return rc;
+        tau_use = tau_cell;
+    }
+    // a3
+    const int32_t mode = closure == 0 ? 1 : 0;
+    const int32_t stride = mode ? 29 : 13;
+    if ((rc = fp_cell_moments(ctx, np, vx_b, vy_b, vz_b, cell_start, mode, mom, stream)) != FP_OK) return rc;
+    // a4 | a5
+    if (closure == 0) rc = fp_closure_exact(ctx, mom, tau_use, coef, flags, nullptr, stream);
+    else              rc = fp_closure_mlp(ctx, mom, stride, tau_use, h_mlp, relax_w, coef, flags, stream);
+    if (rc != FP_OK) return rc;
+    // a6
+    return fp_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, stream);
+}
+
+static int fp_host_stage_alloc(fp_ctx* c)
+{
+    if (c->hs_ready) return FP_OK;
+    const size_t n = (size_t)(c->p.max_particles > 0 ? c->p.max_particles : 1);
+    for (int s = 0; s < 2; ++s) {
+        for (int k = 0; k < 5; ++k) FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_f[s][k], n * 4));
+        FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_pid[s], n * 4));
+    }
+    FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_mom, (size_t)c->ncell * 29 * 8));
+    FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_coef, (size_t)c->ncell * 9 * 4));
+    FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_flags, (size_t)c->ncell * 4));
+    FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_cell_start, ((size_t)c->ncell + 1) * 4));
+    c->hs_ready = true;
+    return FP_OK;
+}
+
+extern "C" int fp_step_host(fp_ctx* ctx, int64_t np,
+                            float* h_x, float* h_y, float* h_vx, float* h_vy, float* h_vz, uint32_t* h_pid,
+                            int32_t closure, const fp_mlp* h_mlp, float relax_w, uint64_t step,
+                            float* h_coef, uint32_t* h_flags, int32_t* h_cell_start, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    if (np < 0 || np > ctx->p.max_particles) return fp_fail(ctx, FP_ERR_STATE, "fp_step_host: np out of range");
+    if (np > 0 && (!h_x || !h_y || !h_vx || !h_vy || !h_vz || !h_pid)) return fp_fail(ctx, FP_ERR_ARG, "fp_step_host: null host pointer");
+    int rc = fp_host_stage_alloc(ctx);
+    if (rc != FP_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    float* hp[5] = {h_x, h_y, h_vx, h_vy, h_vz};
+    const size_t nb = (size_t)np * 4;
+    for (int k = 0; k < 5; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_f[0][k], hp[k], nb, cudaMemcpyHostToDevice, st));
+    if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_pid[0], h_pid, nb, cudaMemcpyHostToDevice, st));
+    rc = fp_step(ctx, np, ctx->hs_f[0][0], ctx->hs_f[0][1], ctx->hs_f[0][2], ctx->hs_f[0][3], ctx->hs_f[0][4], ctx->hs_pid[0],
+                 ctx->hs_f[1][0], ctx->hs_f[1][1], ctx->hs_f[1][2], ctx->hs_f[1][3], ctx->hs_f[1][4], ctx->hs_pid[1],
+                 closure, h_mlp, relax_w, 0, 0.f, nullptr, step, ctx->hs_mom, ctx->hs_coef, ctx->hs_flags,
+                 ctx->hs_cell_start, stream);
+    if (rc != FP_OK) return rc;
+    for (int k = 0; k < 5; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(hp[k], ctx->hs_f[1][k], nb, cudaMemcpyDeviceToHost, st));
+    if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_pid, ctx->hs_pid[1], nb, cudaMemcpyDeviceToHost, st));
+    if (h_coef) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_coef, ctx->hs_coef, (size_t)ctx->ncell * 9 * 4, cudaMemcpyDeviceToHost, st));
+    if (h_flags) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_flags, ctx->hs_flags, (size_t)ctx->ncell * 4, cudaMemcpyDeviceToHost, st));
+    if (h_cell_start) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_cell_start, ctx->hs_cell_start, ((size_t)ctx->ncell + 1) * 4, cudaMemcpyDeviceToHost, st));
+    FP_CUDA_OK(ctx, cudaStreamSynchronize(st));
+    return FP_OK;
+}

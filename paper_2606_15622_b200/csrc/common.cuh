@@ -1,0 +1,159 @@
+// common.cuh -- context, launch helpers and small device utilities shared by the fpcl kernels (sm_100a).
+// Product code: shares nothing with oracle/ (test infrastructure).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/fpcl.h"
+
+#define FPCL_MAX_LAYERS 8
+#define FPCL_NUM_SMS_DEFAULT 148
+
+// ---------------------------------------------------------------------------------------------------------
+// Context.  Owns scratch only (include/fpcl.h "Conventions").
+// ---------------------------------------------------------------------------------------------------------
+struct fp_mlp_dev {                 // uploaded copy of the caller's MLP (fp_closure_mlp caches it)
+    int32_t  n_layers = 0;
+    int32_t  dims[FPCL_MAX_LAYERS + 1] = {0};
+    int32_t  act = 0, feature_set = 0;
+    float    n_scale = 1.f, theta_ref = 0.5f;
+    float*   blob = nullptr;        // device: [W0 | b0 | W1 | b1 | ... | x_mean | x_scale | y_mean | y_scale]
+    size_t   blob_floats = 0;
+    size_t   w_off[FPCL_MAX_LAYERS] = {0}, b_off[FPCL_MAX_LAYERS] = {0};
+    size_t   xm_off = 0, xs_off = 0, ym_off = 0, ys_off = 0;
+    // identity of the source, to skip re-uploading
+    const void* src_W[FPCL_MAX_LAYERS] = {nullptr};
+    const void* src_b[FPCL_MAX_LAYERS] = {nullptr};
+    const void* src_x_mean = nullptr;
+    bool     valid = false;
+};
+
+struct fp_ctx {
+    fp_params p;
+    int32_t   ncell = 0;
+    int32_t   key_bits = 0;         // bits needed for keys in [0, ncell)
+    float     inv_dx = 0.f, inv_dy = 0.f;
+    float     xmin = 0.f, xmax = 0.f, ymin = 0.f, ymax = 0.f, xmax_in = 0.f, ymax_in = 0.f, Lx = 0.f, Ly = 0.f;
+    int       device = 0, num_sms = FPCL_NUM_SMS_DEFAULT;
+    // sort scratch (sized for max_particles)
+    uint32_t *key_a = nullptr, *key_b = nullptr, *idx_a = nullptr, *idx_b = nullptr;
+    uint32_t *block_hist = nullptr;  // [bins][nblocks]
+    uint32_t *bin_total = nullptr;   // [bins]
+    size_t    block_hist_elems = 0;
+    // fp_step_host staging (allocated lazily)
+    float    *hs_f[2][5] = {{nullptr}};
+    uint32_t *hs_pid[2] = {nullptr, nullptr};
+    double   *hs_mom = nullptr;
+    float    *hs_coef = nullptr;
+    uint32_t *hs_flags = nullptr;
+    int32_t  *hs_cell_start = nullptr;
+    bool      hs_ready = false;
+    fp_mlp_dev mlp;
+    char      err[512];
+};
+
+static inline int fp_fail(fp_ctx* ctx, int code, const char* msg)
+{
+    if (ctx) { snprintf(ctx->err, sizeof(ctx->err), "%s", msg); }
+    return code;
+}
+
+#define FP_CUDA_OK(ctx, call)                                                                        \
+    do {                                                                                             \
+        cudaError_t e__ = (call);                                                                    \
+        if (e__ != cudaSuccess) {                                                                    \
+            if (ctx) snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, \
+                              cudaGetErrorString(e__));                                              \
+            return FP_ERR_CUDA;                                                                      \
+        }                                                                                            \
+    } while (0)
+
+#define FP_LAUNCH_OK(ctx) FP_CUDA_OK(ctx, cudaGetLastError())
+
+static inline int fp_div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// internal entry points shared between translation units (not exported)
+int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
+                       const float* x, const float* y, const float* vx, const float* vy, const float* vz,
+                       const uint32_t* pid, float* x_out, float* y_out, float* vx_out, float* vy_out,
+                       float* vz_out, uint32_t* pid_out, int32_t* cell_start, uint32_t* perm, cudaStream_t st);
+int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
+                     const uint32_t* pid, uint64_t step, uint32_t* keys_out /* nullable */, cudaStream_t st);
+int fpi_tau_from_counts(fp_ctx* ctx, const int32_t* cell_start, float tau_ref_n, float* tau_cell, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------------------
+// Device helpers
+// ---------------------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+
+// Cell index along one axis (R1): clamp(floorf((p - p0) * inv_d), 0, n-1), NaN -> 0.
+// (p - p0) * inv_d is a subtract feeding a multiply: no FMA contraction is possible.
+__device__ __forceinline__ int32_t fpd_axis_index(float p, float p0, float inv_d, int32_t n)
+{
+    float t = floorf(__fmul_rn(__fsub_rn(p, p0), inv_d));
+    if (!(t >= 0.0f)) return 0;
+    if (t >= (float)n) return n - 1;
+    return (int32_t)t;
+}
+
+// Philox4x32-10 (Salmon et al., SC'11; R6).  counter (c0..c3), key (k0,k1).
+__device__ __forceinline__ uint4 fpd_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                   uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// word -> uniform in (0,1): ((w >> 9) + 0.5) * 2^-23, exact in fp32.
+// [1,2) mantissa trick: as_float(0x3f800000 | (w>>9)) = 1 + k 2^-23; minus (1 - 2^-24) is exact.
+__device__ __forceinline__ float fpd_uniform(uint32_t w)
+{
+    return __uint_as_float(0x3f800000u | (w >> 9)) - 0.99999994039536f;   // 1 - 2^-24
+}
+
+// 64-bit shuffle helpers
+__device__ __forceinline__ double fpd_shfl_xor(double v, int mask)
+{
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_xor_sync(0xffffffffu, lo, mask);
+    hi = __shfl_xor_sync(0xffffffffu, hi, mask);
+    return __hiloint2double(hi, lo);
+}
+__device__ __forceinline__ double fpd_shfl(double v, int src)
+{
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_sync(0xffffffffu, lo, src);
+    hi = __shfl_sync(0xffffffffu, hi, src);
+    return __hiloint2double(hi, lo);
+}
+
+// Transposing ("multi-value") butterfly over a group of G lanes (G a power of two, groups aligned).
+// In:  v[0..NP) per lane (NP a power of two, NP >= G).  Out: v[0..NP/G) of lane L (L = lane index inside the
+// group) holds the group sum of original slots (NP/G)*L + i.  (NP - NP/G) 64-bit shuffles instead of NP*log2(G).
+template <int NP, int G>
+__device__ __forceinline__ void fpd_transpose_reduce(double (&v)[NP], int lane_in_group)
+{
+    static_assert((NP & (NP - 1)) == 0 && (G & (G - 1)) == 0 && NP >= G, "powers of two");
+#pragma unroll
+    for (int half = G / 2, n = NP; half >= 1; half >>= 1, n >>= 1) {
+        const bool up = (lane_in_group & half) != 0;
+        const int h = n >> 1;
+#pragma unroll
+        for (int i = 0; i < h; ++i) {
+            const double send = up ? v[i] : v[i + h];
+            const double keep = up ? v[i + h] : v[i];
+            v[i] = keep + fpd_shfl_xor(send, half);
+        }
+    }
+}
+
+#endif  // __CUDACC__

@@ -1,0 +1,242 @@
+// sort.cu -- a2: cell key + STABLE sort by key + payload permute + cell_start (
+// DESIGN.md R1).  Integer work: results are bit-exact and unique (equal keys keep input order).
+//
+// Least-significant-digit radix sort on (key, index) pairs, digit width <= 9 bits so that a 2^18-cell grid sorts
+// in two passes.  Each pass = per-tile digit histogram -> per-digit scan over tiles -> stable scatter.  Stability
+// inside a tile comes from warp-striped item order plus __match_any_sync ranking (no atomics decide an order).
+// The payload (x, y, vx, vy, vz, pid) is gathered once at the end through the final permutation.
+#include "common.cuh"
+
+#define SORT_THREADS 256
+#define SORT_WARPS (SORT_THREADS / 32)
+#define SORT_ITEMS 8                                     // items per thread
+#define SORT_TILE (SORT_THREADS * SORT_ITEMS)            // 2048 items per block
+#define SORT_MAX_BINS 512
+
+__global__ void __launch_bounds__(256)
+key_kernel(int64_t np, const float* __restrict__ x, const float* __restrict__ y, uint32_t* __restrict__ keys,
+           int32_t nx, int32_t ny, float x0, float y0, float inv_dx, float inv_dy)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += stride) {
+        const int32_t ix = fpd_axis_index(x[p], x0, inv_dx, nx);
+        const int32_t iy = (ny > 1) ? fpd_axis_index(y[p], y0, inv_dy, ny) : 0;
+        keys[p] = (uint32_t)(iy * nx + ix);
+    }
+}
+
+// per-tile digit histogram: block_hist[bin * nblocks + block]
+__global__ void __launch_bounds__(SORT_THREADS)
+hist_kernel(int64_t np, const uint32_t* __restrict__ keys, uint32_t* __restrict__ block_hist, int nblocks,
+            int shift, int bins)
+{
+    __shared__ uint32_t h[SORT_MAX_BINS];
+    for (int b = threadIdx.x; b < bins; b += SORT_THREADS) h[b] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+    const uint32_t mask = (uint32_t)bins - 1u;
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        const int64_t p = base + i * SORT_THREADS + threadIdx.x;
+        if (p < np) atomicAdd(&h[(keys[p] >> shift) & mask], 1u);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < bins; b += SORT_THREADS) block_hist[(size_t)b * nblocks + blockIdx.x] = h[b];
+}
+
+// one warp per digit value: exclusive scan of that digit's counts over tiles (in place) and the digit total
+__global__ void __launch_bounds__(128)
+scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_total, int nblocks, int bins)
+{
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= bins) return;
+    uint32_t* row = block_hist + (size_t)warp * nblocks;
+    uint32_t carry = 0;
+    for (int b0 = 0; b0 < nblocks; b0 += 32) {
+        const int b = b0 + lane;
+        const uint32_t v = (b < nblocks) ? row[b] : 0u;
+        uint32_t s = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, s, d); if (lane >= d) s += t; }
+        if (b < nblocks) row[b] = carry + s - v;
+        carry += __shfl_sync(0xffffffffu, s, 31);
+    }
+    if (lane == 0) bin_total[warp] = carry;
+}
+
+// stable scatter of one tile.  Warp w owns items [w*256, (w+1)*256) of the tile in warp-striped order
+// (round i, lane l -> w*256 + i*32 + l), so (tile, warp, round, lane) order is input order.
+template <bool FIRST_PASS>
+__global__ void __launch_bounds__(SORT_THREADS)
+scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
+               uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out,
+               const uint32_t* __restrict__ block_hist, const uint32_t* __restrict__ bin_total, int nblocks,
+               int shift, int bins)
+{
+    __shared__ uint32_t cnt[SORT_WARPS][SORT_MAX_BINS];   // per-warp running digit counts, then bases
+    __shared__ uint32_t bin_base[SORT_MAX_BINS];          // global start of each digit value + this tile's offset
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t mask = (uint32_t)bins - 1u;
+    for (int b = threadIdx.x; b < bins * SORT_WARPS; b += SORT_THREADS) (&cnt[0][0])[(b / bins) * SORT_MAX_BINS + (b % bins)] = 0;
+    // exclusive scan of the digit totals (bins <= 512) by warp 0, two elements per pass
+    if (warp == 0) {
+        uint32_t carry = 0;
+        for (int b0 = 0; b0 < bins; b0 += 32) {
+            const int b = b0 + lane;
+            const uint32_t v = (b < bins) ? bin_total[b] : 0u;
+            uint32_t s = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, s, d); if (lane >= d) s += t; }
+            if (b < bins) bin_base[b] = carry + s - v + block_hist[(size_t)b * nblocks + blockIdx.x];
+            carry += __shfl_sync(0xffffffffu, s, 31);
+        }
+    }
+    __syncthreads();
+    const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS);
+    uint32_t key[SORT_ITEMS], idx[SORT_ITEMS], rank[SORT_ITEMS];
+    bool valid[SORT_ITEMS];
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        const int64_t p = wbase + i * 32 + lane;
+        valid[i] = p < np;
+        key[i] = valid[i] ? keys_in[p] : 0xffffffffu;
+        idx[i] = FIRST_PASS ? (uint32_t)p : (valid[i] ? idx_in[p] : 0u);
+    }
+    // rank inside the warp's sub-tile, round by round (stable)
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        const uint32_t d = (key[i] >> shift) & mask;
+        const uint32_t act = __ballot_sync(0xffffffffu, valid[i]);
+        uint32_t r = 0;
+        if (valid[i]) {
+            const uint32_t peers = __match_any_sync(act, d);
+            const int leader = __ffs(peers) - 1;
+            const uint32_t before = __popc(peers & ((1u << lane) - 1u));
+            uint32_t c = 0;
+            if (lane == leader) { c = cnt[warp][d]; cnt[warp][d] = c + __popc(peers); }
+            c = __shfl_sync(peers, c, leader);
+            r = c + before;
+        }
+        rank[i] = r;
+        __syncwarp();
+    }
+    __syncthreads();
+    // per digit value: exclusive scan over the warps -> base of (warp, digit) inside the tile's digit run
+    for (int b = threadIdx.x; b < bins; b += SORT_THREADS) {
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) { const uint32_t c = cnt[w][b]; cnt[w][b] = run; run += c; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        if (valid[i]) {
+            const uint32_t d = (key[i] >> shift) & mask;
+            const uint32_t dst = bin_base[d] + cnt[warp][d] + rank[i];
+            keys_out[dst] = key[i];
+            idx_out[dst] = idx[i];
+        }
+    }
+}
+
+// cell_start from the sorted keys: cell_start[k] = first position whose key >= k; cell_start[ncell] = np.
+__global__ void __launch_bounds__(256)
+cell_start_kernel(int64_t np, const uint32_t* __restrict__ skeys, int32_t ncell, int32_t* __restrict__ cell_start)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p <= np; p += stride) {
+        const int64_t lo = (p == 0) ? 0 : (int64_t)skeys[p - 1] + 1;
+        const int64_t hi = (p == np) ? (int64_t)ncell : (int64_t)skeys[p];
+        for (int64_t k = lo; k <= hi; ++k) cell_start[k] = (int32_t)p;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+gather_kernel(int64_t np, const uint32_t* __restrict__ perm,
+              const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ vx,
+              const float* __restrict__ vy, const float* __restrict__ vz, const uint32_t* __restrict__ pid,
+              float* __restrict__ xo, float* __restrict__ yo, float* __restrict__ vxo, float* __restrict__ vyo,
+              float* __restrict__ vzo, uint32_t* __restrict__ pido)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < np; k += stride) {
+        const uint32_t s = perm[k];
+        xo[k] = x[s]; yo[k] = y[s]; vxo[k] = vx[s]; vyo[k] = vy[s]; vzo[k] = vz[s]; pido[k] = pid[s];
+    }
+}
+
+__global__ void zero_i32_kernel(int32_t* a, int64_t n)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] = 0;
+}
+
+int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
+                       const float* x, const float* y, const float* vx, const float* vy, const float* vz,
+                       const uint32_t* pid, float* x_out, float* y_out, float* vx_out, float* vy_out,
+                       float* vz_out, uint32_t* pid_out, int32_t* cell_start, uint32_t* perm, cudaStream_t st)
+{
+    const int32_t ncell = ctx->ncell;
+    if (np == 0) {
+        zero_i32_kernel<<<fp_div_up(ncell + 1, 256), 256, 0, st>>>(cell_start, (int64_t)ncell + 1);
+        FP_LAUNCH_OK(ctx);
+        return FP_OK;
+    }
+    const int nblocks = fp_div_up(np, SORT_TILE);
+    const int bits = ctx->key_bits < 1 ? 1 : ctx->key_bits;
+    const int passes = (bits + 8) / 9;
+    const int dbits = (bits + passes - 1) / passes;          // <= 9
+    const int bins = 1 << dbits;
+    if ((size_t)bins * nblocks > ctx->block_hist_elems) return fp_fail(ctx, FP_ERR_STATE, "sort scratch too small");
+    const uint32_t* kin = keys;
+    const uint32_t* iin = nullptr;
+    uint32_t* kout = ctx->key_a;
+    uint32_t* iout = ctx->idx_a;
+    for (int pass = 0; pass < passes; ++pass) {
+        const int shift = pass * dbits;
+        hist_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, kin, ctx->block_hist, nblocks, shift, bins);
+        scan_rows_kernel<<<fp_div_up((int64_t)bins * 32, 128), 128, 0, st>>>(ctx->block_hist, ctx->bin_total, nblocks, bins);
+        if (pass == 0)
+            scatter_kernel<true><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, ctx->block_hist, ctx->bin_total, nblocks, shift, bins);
+        else
+            scatter_kernel<false><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, ctx->block_hist, ctx->bin_total, nblocks, shift, bins);
+        FP_LAUNCH_OK(ctx);
+        kin = kout; iin = iout;
+        kout = (kout == ctx->key_a) ? ctx->key_b : ctx->key_a;
+        iout = (iout == ctx->idx_a) ? ctx->idx_b : ctx->idx_a;
+    }
+    const int64_t cap = (int64_t)ctx->num_sms * 16;
+    int64_t want = (np + 1 + 255) / 256;
+    cell_start_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, kin, ncell, cell_start);
+    want = (np + 255) / 256;
+    gather_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, iin, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out, pid_out);
+    FP_LAUNCH_OK(ctx);
+    if (perm) FP_CUDA_OK(ctx, cudaMemcpyAsync(perm, iin, (size_t)np * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
+    return FP_OK;
+}
+
+extern "C" int fp_sort_by_cell(fp_ctx* ctx, int64_t np,
+                               const float* x, const float* y, const float* vx, const float* vy, const float* vz,
+                               const uint32_t* pid,
+                               float* x_out, float* y_out, float* vx_out, float* vy_out, float* vz_out,
+                               uint32_t* pid_out, int32_t* cell_start, uint32_t* perm, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    if (np < 0 || !cell_start) return fp_fail(ctx, FP_ERR_ARG, "fp_sort_by_cell: np < 0 or null cell_start");
+    if (np > ctx->p.max_particles) return fp_fail(ctx, FP_ERR_STATE, "fp_sort_by_cell: np > max_particles");
+    if (np > 0 && (!x || !y || !vx || !vy || !vz || !pid || !x_out || !y_out || !vx_out || !vy_out || !vz_out || !pid_out))
+        return fp_fail(ctx, FP_ERR_ARG, "fp_sort_by_cell: null pointer");
+    if (np > 0 && (x == x_out || y == y_out || vx == vx_out || vy == vy_out || vz == vz_out || pid == pid_out))
+        return fp_fail(ctx, FP_ERR_ARG, "fp_sort_by_cell: outputs may not alias inputs");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (np > 0) {
+        const fp_params& q = ctx->p;
+        const int64_t cap = (int64_t)ctx->num_sms * 16;
+        const int64_t want = (np + 255) / 256;
+        key_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, x, y, ctx->key_b, q.nx, q.ny, q.x0, q.y0, ctx->inv_dx, ctx->inv_dy);
+        FP_LAUNCH_OK(ctx);
+    }
+    // keys live in key_b; the first pass writes key_a, so the ping-pong never overwrites its own input
+    return fpi_sort_with_keys(ctx, np, ctx->key_b, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out,
+                              pid_out, cell_start, perm, st);
+}

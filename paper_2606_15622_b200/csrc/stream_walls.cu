@@ -1,0 +1,148 @@
+// stream_walls.cu -- a0 + a1: streaming (Eq. 16 :187) and diffuse isothermal walls (:214, :380, :674;
+// DESIGN.md R7), fused with the cell-key computation of a2 (R1) when called from fp_step.
+//
+// One thread per particle, SoA fp32, fully coalesced: 24 B read (x, y, vx, vy, vz, pid is read only by particles
+// that hit a wall), 8 B written (x, y) + 4 B key; wall hits add 12 B of velocity writes.  HBM-bound.
+// Positions follow a fixed fp32 operation sequence (they decide the integer cell index); re-emitted velocities
+// are drawn with fp32 logf / sincospif from the Philox uniforms (tolerance 1e-6 relative).
+#include "common.cuh"
+
+struct sw_params {
+    int32_t nx, ny;
+    float x0, y0, inv_dx, inv_dy, dt;
+    float xmin, xmax, ymin, ymax, xmax_in, ymax_in, Lx, Ly;
+    fp_wall wall[4];
+    int32_t body_kind;
+    float bcx, bcy, bR, bR_out, bR2, body_theta_w;
+    uint32_t k0, k1, step_lo, step_hi;
+};
+
+// One wall draw (R7): normal component sqrt(-2 theta_w ln u0) into the gas, tangentials
+// sqrt(theta_w) * sqrt(-2 ln u1) * (cos, sin)(2 pi u2).
+__device__ __forceinline__ void sw_wall_draw(const sw_params& P, uint32_t pid, uint32_t stream, float theta_w,
+                                             float& vn, float& t1, float& t2)
+{
+    const uint4 w = fpd_philox4x32_10(pid, P.step_lo, P.step_hi, stream, P.k0, P.k1);
+    const float u0 = fpd_uniform(w.x), u1 = fpd_uniform(w.y), u2 = fpd_uniform(w.z);
+    vn = sqrtf(-2.0f * theta_w * logf(u0));
+    const float r = sqrtf(theta_w) * sqrtf(-2.0f * logf(u1));
+    float s, c;
+    sincospif(2.0f * u2, &s, &c);
+    t1 = r * c;
+    t2 = r * s;
+}
+
+template <bool WRITE_KEYS>
+__global__ void __launch_bounds__(256)
+sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
+          float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
+          uint32_t* __restrict__ keys, const __grid_constant__ sw_params P)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += stride) {
+        float v0 = vx[p], v1 = vy[p], v2 = vz[p];
+        float xp = fmaf(v0, P.dt, x[p]);
+        float yp = fmaf(v1, P.dt, y[p]);
+        bool redrawn = false;
+        // x pair
+        {
+            const int side = (xp < P.xmin) ? 0 : ((xp >= P.xmax) ? 1 : -1);
+            if (side >= 0) {
+                const fp_wall w = P.wall[side];
+                const float xw = side ? P.xmax : P.xmin;
+                if (w.kind == FP_WALL_DIFFUSE) {
+                    xp = __fadd_rn(xw, __fsub_rn(xw, xp));
+                    if (xp < P.xmin) xp = P.xmin;
+                    if (xp >= P.xmax) xp = P.xmax_in;
+                    float vn, t1, t2;
+                    sw_wall_draw(P, pid[p], 1u, w.theta_w, vn, t1, t2);
+                    v0 = side ? -vn : vn; v1 = w.uy + t1; v2 = w.uz + t2; redrawn = true;
+                } else if (w.kind == FP_WALL_PERIODIC) {
+                    xp = side ? __fsub_rn(xp, P.Lx) : __fadd_rn(xp, P.Lx);
+                    if (xp < P.xmin) xp = P.xmin;
+                    if (xp >= P.xmax) xp = P.xmax_in;
+                }
+            }
+        }
+        // y pair
+        if (P.ny > 1) {
+            const int side = (yp < P.ymin) ? 0 : ((yp >= P.ymax) ? 1 : -1);
+            if (side >= 0) {
+                const fp_wall w = P.wall[2 + side];
+                const float yw = side ? P.ymax : P.ymin;
+                if (w.kind == FP_WALL_DIFFUSE) {
+                    yp = __fadd_rn(yw, __fsub_rn(yw, yp));
+                    if (yp < P.ymin) yp = P.ymin;
+                    if (yp >= P.ymax) yp = P.ymax_in;
+                    float vn, t1, t2;
+                    sw_wall_draw(P, pid[p], 2u, w.theta_w, vn, t1, t2);
+                    v1 = side ? -vn : vn; v0 = w.ux + t1; v2 = w.uz + t2; redrawn = true;
+                } else if (w.kind == FP_WALL_PERIODIC) {
+                    yp = side ? __fsub_rn(yp, P.Ly) : __fadd_rn(yp, P.Ly);
+                    if (yp < P.ymin) yp = P.ymin;
+                    if (yp >= P.ymax) yp = P.ymax_in;
+                }
+            }
+        }
+        // embedded body: a particle inside the cylinder is moved radially to R (1 + 1e-6) and re-emitted
+        if (P.body_kind == 1) {
+            const float ddx = __fsub_rn(xp, P.bcx), ddy = __fsub_rn(yp, P.bcy);
+            const float r2 = fmaf(ddy, ddy, __fmul_rn(ddx, ddx));
+            if (r2 < P.bR2) {
+                const float r = sqrtf(r2);
+                float nxn, nyn;
+                if (r > 0.0f) {
+                    const float sc = __fdiv_rn(P.bR_out, r);
+                    nxn = ddx / r; nyn = ddy / r;
+                    xp = fmaf(ddx, sc, P.bcx); yp = fmaf(ddy, sc, P.bcy);
+                } else { nxn = 1.0f; nyn = 0.0f; xp = __fadd_rn(P.bcx, P.bR_out); }
+                float vn, t1, t2;
+                sw_wall_draw(P, pid[p], 4u, P.body_theta_w, vn, t1, t2);
+                v0 = vn * nxn - t1 * nyn; v1 = vn * nyn + t1 * nxn; v2 = t2; redrawn = true;
+            }
+        }
+        x[p] = xp; y[p] = yp;
+        if (redrawn) { vx[p] = v0; vy[p] = v1; vz[p] = v2; }
+        if (WRITE_KEYS) {
+            const int32_t ix = fpd_axis_index(xp, P.x0, P.inv_dx, P.nx);
+            const int32_t iy = (P.ny > 1) ? fpd_axis_index(yp, P.y0, P.inv_dy, P.ny) : 0;
+            keys[p] = (uint32_t)(iy * P.nx + ix);
+        }
+    }
+}
+
+int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
+                     const uint32_t* pid, uint64_t step, uint32_t* keys_out, cudaStream_t st)
+{
+    if (np == 0) return FP_OK;
+    const fp_params& q = ctx->p;
+    sw_params P;
+    P.nx = q.nx; P.ny = q.ny; P.x0 = q.x0; P.y0 = q.y0; P.inv_dx = ctx->inv_dx; P.inv_dy = ctx->inv_dy; P.dt = q.dt;
+    P.xmin = ctx->xmin; P.xmax = ctx->xmax; P.ymin = ctx->ymin; P.ymax = ctx->ymax;
+    P.xmax_in = ctx->xmax_in; P.ymax_in = ctx->ymax_in; P.Lx = ctx->Lx; P.Ly = ctx->Ly;
+    for (int k = 0; k < 4; ++k) P.wall[k] = q.wall[k];
+    P.body_kind = q.body_kind; P.bcx = q.body_cx; P.bcy = q.body_cy; P.bR = q.body_R;
+    {   // fp32, two separate roundings (the host compiler targets baseline x86-64: no FMA contraction)
+        volatile float rout = q.body_R * 1.000001f; P.bR_out = rout;
+        volatile float r2 = q.body_R * q.body_R;    P.bR2 = r2;
+    }
+    P.body_theta_w = q.body_theta_w;
+    P.k0 = (uint32_t)q.seed; P.k1 = (uint32_t)(q.seed >> 32);
+    P.step_lo = (uint32_t)step; P.step_hi = (uint32_t)(step >> 32);
+    const int threads = 256;
+    int64_t want = (np + threads - 1) / threads;
+    const int64_t cap = (int64_t)ctx->num_sms * 16;
+    const int blocks = (int)(want < cap ? want : cap);
+    if (keys_out) sw_kernel<true><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, keys_out, P);
+    else          sw_kernel<false><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, nullptr, P);
+    FP_LAUNCH_OK(ctx);
+    return FP_OK;
+}
+
+extern "C" int fp_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
+                               const uint32_t* pid, uint64_t step, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    if (np < 0 || (np > 0 && (!x || !y || !vx || !vy || !vz || !pid))) return fp_fail(ctx, FP_ERR_ARG, "fp_stream_walls: null pointer or np < 0");
+    return fpi_stream_walls(ctx, np, x, y, vx, vy, vz, pid, step, nullptr, (cudaStream_t)stream);
+}

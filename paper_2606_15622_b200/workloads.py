@@ -240,3 +240,29 @@ def xavier_mlp(dims=(13, 64, 64, 64, 9), seed=0, act=0, feature_set=0, n_scale=0
                 x_scale=np.array(x_scale, dtype=np.float32), y_mean=y_mean, y_scale=y_scale, act=int(act),
                 feature_set=int(feature_set), n_scale=float(np.float32(n_scale)),
                 theta_ref=float(np.float32(theta_ref)))
+
+
+# ------------------------------------------------------------------------------------------------ ragged test case
+def ragged(nx=37, ny=23, seed=7, mean_ppc=40.0, empty_frac=0.1, shuffle=True, walls=None, drift=0.0):
+    """Edge-case ensemble for parity tests: per-cell counts 0..~4x mean (about ``empty_frac`` empty cells, some
+    cells with 1-3 particles, a few very full ones), per-cell bulk velocity (+ ``drift`` on x) and temperature."""
+    rng = _rng(seed)
+    nc = nx * ny
+    dx, dy = 1.0 / nx, 1.0 / ny
+    lam = mean_ppc * rng.gamma(2.0, 0.5, size=nc)
+    counts = rng.poisson(lam)
+    counts[rng.uniform(size=nc) < empty_frac] = 0
+    small = rng.uniform(size=nc) < 0.05
+    counts[small] = rng.integers(1, 4, size=int(small.sum()))
+    big = rng.integers(0, nc, size=3)
+    counts[big] = (mean_ppc * rng.integers(8, 14, size=3)).astype(np.int64)
+    cfg = make_config(nx, ny, dx, dy, 0.02, 0.7, walls or NO_WALLS, seed=seed, max_particles=int(counts.sum()))
+    x, y, cell = _positions_in_cells(rng, counts, nx, ny, dx, dy)
+    n = x.shape[0]
+    th = rng.uniform(0.2, 1.5, size=nc)[cell]
+    U = rng.uniform(-0.5, 0.5, size=(nc, 3))[cell]
+    U[:, 0] += drift
+    v = U + rng.normal(size=(n, 3)) * np.sqrt(th)[:, None]
+    # skew the distribution a little so that odd moments are not pure noise
+    v += 0.15 * (rng.exponential(size=(n, 3)) - 1.0) * np.sqrt(th)[:, None]
+    return cfg, _finish(rng, x, y, v, shuffle)

@@ -1,0 +1,247 @@
+"""GPU-vs-oracle parity, stage by stage, through the C ABI (include/fpcl.h) on the same seeded inputs.
+
+Integer work (cell keys, sort order, cell_start, streamed positions) must match bit for bit; floating point within
+the tolerances of BASELINE.json's north_star as read in tests/parity_util.py / DESIGN.md.
+"""
+import numpy as np
+import pytest
+
+from parity_util import coef_ratio, moment_ratio, velocity_ratio
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_15622_b200 import fpcl
+    fpcl.load()
+    return fpcl
+
+
+@pytest.fixture(scope="module")
+def wl():
+    from paper_2606_15622_b200 import workloads
+    return workloads
+
+
+def _cases(wl):
+    c1 = wl.couette()
+    rg = wl.ragged()
+    rg2 = wl.ragged(nx=64, ny=1, seed=11, mean_ppc=150.0)
+    cav = wl.cavity(n=24, ppc=30, seed=5)
+    return {"couette": c1, "ragged": rg, "ragged1d": rg2, "cavity24": cav}
+
+
+# ------------------------------------------------------------------------------------------------ a2 sort
+@pytest.mark.parametrize("name", ["couette", "ragged", "ragged1d", "cavity24"])
+def test_sort_bit_exact(gpu, wl, orc, name):
+    cfg, st = _cases(wl)[name]
+    ref, ref_cs, ref_perm = orc.sort_by_cell(st, cfg)
+    ctx = gpu.Context(cfg)
+    out, cs, perm = ctx.sort_by_cell(gpu.to_device(st))
+    got = gpu.to_host(out)
+    assert np.array_equal(cs.cpu().numpy(), ref_cs)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), ref_perm)
+    for k in ("x", "y", "vx", "vy", "vz", "pid"):
+        assert np.array_equal(got[k].view(np.uint32), ref[k].view(np.uint32)), k
+    ctx.close()
+
+
+def test_sort_edge_positions(gpu, wl, orc):
+    """Out-of-domain, boundary and NaN positions clamp exactly as the oracle; many ties; np = 0 and 1."""
+    cfg, st = wl.ragged(nx=19, ny=7, seed=3, mean_ppc=20.0)
+    rng = np.random.default_rng(0)
+    n = st["x"].shape[0]
+    idx = rng.choice(n, size=200, replace=False)
+    st["x"][idx[:40]] = -0.5
+    st["x"][idx[40:80]] = 1.0
+    st["x"][idx[80:100]] = np.float32(1.0) + np.float32(1e-3)
+    st["y"][idx[100:140]] = np.nan
+    st["y"][idx[140:170]] = np.float32(np.nextafter(np.float32(1.0), np.float32(0.0)))
+    st["x"][idx[170:200]] = (np.arange(30) % 19) / np.float32(19.0)     # exact cell edges
+    ref, ref_cs, ref_perm = orc.sort_by_cell(st, cfg)
+    ctx = gpu.Context(cfg)
+    out, cs, perm = ctx.sort_by_cell(gpu.to_device(st))
+    assert np.array_equal(cs.cpu().numpy(), ref_cs)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), ref_perm)
+    for m in (0, 1):
+        sub = {k: v[:m].copy() for k, v in st.items()}
+        r, rcs, rperm = orc.sort_by_cell(sub, cfg)
+        o, c, p = ctx.sort_by_cell(gpu.to_device(sub))
+        assert np.array_equal(c.cpu().numpy(), rcs)
+        assert np.array_equal(p.cpu().numpy().view(np.uint32), rperm)
+    ctx.close()
+
+
+def test_sort_three_passes(gpu, wl, orc):
+    """More than 2^18 cells forces a third radix pass."""
+    rng = np.random.default_rng(5)
+    nx, ny, n = 1024, 300, 300_000
+    cfg = wl.make_config(nx, ny, 1.0, 1.0, 0.01, 1.0, wl.NO_WALLS, max_particles=n)
+    st = dict(x=rng.uniform(0, nx, n).astype(np.float32), y=rng.uniform(0, ny, n).astype(np.float32),
+              vx=rng.normal(size=n).astype(np.float32), vy=rng.normal(size=n).astype(np.float32),
+              vz=rng.normal(size=n).astype(np.float32), pid=np.arange(n, dtype=np.uint32))
+    ref, ref_cs, ref_perm = orc.sort_by_cell(st, cfg)
+    ctx = gpu.Context(cfg)
+    out, cs, perm = ctx.sort_by_cell(gpu.to_device(st))
+    assert np.array_equal(cs.cpu().numpy(), ref_cs)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), ref_perm)
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ a3 moments
+def _sorted_case(orc, cfg, st):
+    s, cs, _ = orc.sort_by_cell(st, cfg)
+    return s, cs
+
+
+@pytest.mark.parametrize("name", ["couette", "ragged", "ragged1d", "cavity24"])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_moments(gpu, wl, orc, name, mode):
+    import torch
+    cfg, st = _cases(wl)[name]
+    s, cs = _sorted_case(orc, cfg, st)
+    ref = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, mode)
+    ctx = gpu.Context(cfg)
+    d = gpu.to_device(s)
+    mom = ctx.cell_moments(d["vx"], d["vy"], d["vz"], torch.from_numpy(cs).cuda(), mode)
+    r = moment_ratio(mom.cpu().numpy(), ref)
+    print("moments %s mode %d: worst err/allowed = %.3f" % (name, mode, r))
+    assert r <= 1.0
+    ctx.close()
+
+
+def test_moments_mach10_shift(gpu, wl, orc):
+    """Galilean shift of 9.09 c_mp (Mach 10) and of 2624 (raw m/s): central moments must survive."""
+    import torch
+    cfg, st = wl.ragged(nx=30, ny=20, seed=9, mean_ppc=100.0)
+    s, cs = _sorted_case(orc, cfg, st)
+    ctx = gpu.Context(cfg)
+    for shift, scale in ((9.09, 1.0), (2624.0, 288.6)):
+        vx = (s["vx"] * np.float32(scale) + np.float32(shift)).astype(np.float32)
+        vy = (s["vy"] * np.float32(scale)).astype(np.float32)
+        vz = (s["vz"] * np.float32(scale)).astype(np.float32)
+        ref = orc.cell_moments(vx, vy, vz, cs, 1)
+        mom = ctx.cell_moments(torch.from_numpy(vx).cuda(), torch.from_numpy(vy).cuda(), torch.from_numpy(vz).cuda(),
+                               torch.from_numpy(cs).cuda(), 1)
+        r = moment_ratio(mom.cpu().numpy(), ref)
+        print("moments shift %g: worst err/allowed = %.3f" % (shift, r))
+        assert r <= 1.0
+    ctx.close()
+
+
+def test_moments_group_widths(gpu, wl, orc):
+    """Mean particles per cell selects the lane-group width (4, 8, 16): cover all three and one huge cell."""
+    import torch
+    for mean_ppc, seed in ((12.0, 21), (90.0, 22), (260.0, 23)):
+        cfg, st = wl.ragged(nx=16, ny=12, seed=seed, mean_ppc=mean_ppc)
+        s, cs = _sorted_case(orc, cfg, st)
+        ctx = gpu.Context(cfg)
+        d = gpu.to_device(s)
+        for mode in (0, 1):
+            ref = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, mode)
+            mom = ctx.cell_moments(d["vx"], d["vy"], d["vz"], torch.from_numpy(cs).cuda(), mode)
+            r = moment_ratio(mom.cpu().numpy(), ref)
+            print("moments ppc %g mode %d: %.3f" % (mean_ppc, mode, r))
+            assert r <= 1.0
+        ctx.close()
+    # all particles in one cell of a 4-cell grid (chunked accumulation path)
+    rng = np.random.default_rng(4)
+    n = 50_000
+    cfg = wl.make_config(2, 2, 0.5, 0.5, 0.01, 1.0, wl.NO_WALLS, max_particles=n)
+    v = rng.normal(0.3, 0.8, size=(3, n)).astype(np.float32)
+    cs = np.array([0, 0, n, n, n], dtype=np.int32)
+    ref = orc.cell_moments(v[0], v[1], v[2], cs, 1)
+    ctx = gpu.Context(cfg)
+    mom = ctx.cell_moments(torch.from_numpy(v[0]).cuda(), torch.from_numpy(v[1]).cuda(), torch.from_numpy(v[2]).cuda(),
+                           torch.from_numpy(cs).cuda(), 1)
+    assert moment_ratio(mom.cpu().numpy(), ref) <= 1.0
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ a4 exact closure
+def _theta(mom):
+    return (mom[:, 4] + mom[:, 7] + mom[:, 9]) / 3.0
+
+
+@pytest.mark.parametrize("name", ["couette", "ragged", "c2small"])
+def test_closure_exact(gpu, wl, orc, name):
+    import torch
+    if name == "c2small":
+        cfg, st, _ = wl.grad13_cells(ncx=40, ncy=30, ppc=50, seed=1)
+    else:
+        cfg, st = _cases(wl)[name]
+    s, cs = _sorted_case(orc, cfg, st)
+    mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 1)
+    rng = np.random.default_rng(2)
+    for tau in (cfg["tau"], rng.uniform(0.3, 3.0, size=mom.shape[0]).astype(np.float32)):
+        ref, rflags, kappa = orc.closure_exact(mom, tau, cfg["eps2_scale"], cfg["min_count"])
+        ctx = gpu.Context(cfg)
+        tau_d = None if np.ndim(tau) == 0 else torch.from_numpy(tau).cuda()
+        coef, flags, kap = ctx.closure_exact(torch.from_numpy(mom).cuda(), tau_d, want_kappa=True)
+        coef, flags = coef.cpu().numpy(), flags.cpu().numpy().view(np.uint32)
+        hard = orc.FLAG_EMPTY | orc.FLAG_LOWCOUNT | orc.FLAG_SINGULAR
+        assert np.array_equal(flags & hard, rflags & hard)
+        ok = (rflags & orc.FLAG_ILLCOND) == 0
+        r = coef_ratio(coef, ref, tau, _theta(mom), 1e-5, mask=ok)
+        # fallback cells are exact Langevin / zeros
+        fb = (rflags & hard) != 0
+        assert np.allclose(coef[fb], ref[fb].astype(np.float32), rtol=1e-7, atol=0)
+        print("closure_exact %s: worst err/allowed %.3g over %d cells (%d flagged ill-conditioned by the oracle, "
+              "%d by the GPU estimate), kappa max %.3g" % (name, r, int(ok.sum()), int((~ok).sum()),
+                                                        int(((flags & orc.FLAG_ILLCOND) != 0).sum()), kappa.max()))
+        assert r <= 1.0
+        assert np.isfinite(coef).all()
+        ctx.close()
+
+
+def test_closure_exact_langevin(gpu, wl):
+    """Exact Maxwellian moments give c = -delta/tau, gamma = 0 (Eq. 4 :77)."""
+    import torch
+    cfg = wl.make_config(4, 1, 0.25, 1.0, 0.01, 0.8, wl.NO_WALLS, max_particles=16)
+    th = np.array([0.5, 1.0, 2.5, 0.1])
+    mom = np.zeros((4, 29))
+    mom[:, 0] = 100
+    for k in (4, 7, 9):
+        mom[:, k] = th
+    for k in (20, 23, 25):
+        mom[:, k] = 5 * th ** 2
+    ctx = gpu.Context(cfg)
+    coef, flags = ctx.closure_exact(torch.from_numpy(mom).cuda())
+    coef = coef.cpu().numpy()
+    want = np.array([-1 / 0.8, 0, 0, -1 / 0.8, 0, -1 / 0.8, 0, 0, 0])
+    assert np.allclose(coef, want[None, :], rtol=1e-6, atol=1e-7)
+    assert (flags.cpu().numpy() == 0).all()
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ a5 MLP surrogate
+@pytest.mark.parametrize("shape", ["13-64x3-silu", "13-64x3-relu", "16-32-relu", "13-7-5-silu", "16-256x4-relu"])
+@pytest.mark.parametrize("stride", [13, 29])
+def test_closure_mlp(gpu, wl, orc, shape, stride):
+    import torch
+    cfg, st = wl.ragged(nx=25, ny=16, seed=13, mean_ppc=60.0)
+    s, cs = _sorted_case(orc, cfg, st)
+    mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 1 if stride == 29 else 0)
+    dims, act, fs = {"13-64x3-silu": ((13, 64, 64, 64, 9), 0, 0), "13-64x3-relu": ((13, 64, 64, 64, 9), 1, 0),
+                     "16-32-relu": ((16, 32, 9), 1, 1), "13-7-5-silu": ((13, 7, 5, 9), 0, 0),
+                     "16-256x4-relu": ((16, 256, 256, 256, 256, 9), 1, 1)}[shape]
+    mlp = wl.xavier_mlp(dims=dims, seed=0, act=act, feature_set=fs, n_scale=1.0 / 60.0, tau=cfg["tau"], bias_scale=0.1)
+    tau = np.random.default_rng(3).uniform(0.4, 2.0, size=mom.shape[0]).astype(np.float32)
+    ctx = gpu.Context(cfg)
+    dm = gpu.Mlp(mlp)
+    for relax_w in (1.0, 0.2):
+        old = np.random.default_rng(8).normal(size=(mom.shape[0], 9)).astype(np.float32)
+        ref, rflags = orc.closure_mlp(mom, mlp, tau, min_count=cfg["min_count_mlp"], relax_w=relax_w, coef_old=old)
+        coef, flags = ctx.closure_mlp(torch.from_numpy(mom).cuda(), dm, torch.from_numpy(tau).cuda(), relax_w,
+                                      coef=torch.from_numpy(old.copy()).cuda())
+        coef, flags = coef.cpu().numpy(), flags.cpu().numpy().view(np.uint32)
+        assert np.array_equal(flags, rflags)
+        r = coef_ratio(coef, ref, tau, _theta(mom), 1e-5, mask=(rflags & orc.FLAG_EMPTY) == 0)
+        print("closure_mlp %s stride %d w %.1f: worst err/allowed %.3g" % (shape, stride, relax_w, r))
+        assert r <= 1.0
+        assert np.isfinite(coef).all()
+    ctx.close()
