@@ -169,6 +169,17 @@ int fp_step_host(fp_ctx* ctx, int64_t np,
                  int32_t closure, const fp_mlp* h_mlp, float relax_w, uint64_t step,
                  float* h_coef, uint32_t* h_flags, int32_t* h_cell_start, void* stream);
 
+/* Measurement hooks (bench.py).  fp_timing_enable(ctx, max_steps) makes every following fp_step record CUDA events
+ * on the caller's stream at its stage boundaries (max_steps = 0 switches it off and frees the events);
+ * fp_timing_read waits for the last recorded event and writes, for each recorded step, FP_NSTAGES durations in
+ * milliseconds to h_ms (host, [max_steps * FP_NSTAGES]) in the order: stream+walls(+keys), radix sort + cell_start,
+ * payload gather, moment gather, closure, velocity update; *h_nsteps receives the number of steps recorded and the
+ * recorder is reset.  fp_launch_count returns the number of kernels this context has launched so far. */
+#define FP_NSTAGES 6
+int fp_timing_enable(fp_ctx* ctx, int32_t max_steps);
+int fp_timing_read(fp_ctx* ctx, float* h_ms, int32_t* h_nsteps);
+uint64_t fp_launch_count(const fp_ctx* ctx);
+
 #ifdef __cplusplus
 }
 #endif

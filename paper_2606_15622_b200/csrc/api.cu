@@ -21,6 +21,8 @@ static void fp_free_all(fp_ctx* c)
     cudaFree(c->mlp.blob);
 }
 
+static void fp_timing_free(fp_ctx* c);
+
 extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
 {
     if (!out || !h_params) return FP_ERR_ARG;
@@ -67,6 +69,7 @@ extern "C" int fp_destroy(fp_ctx* ctx)
 {
     if (!ctx) return FP_ERR_ARG;
     cudaDeviceSynchronize();
+    fp_timing_free(ctx);
     fp_free_all(ctx);
     delete ctx;
     return FP_OK;
@@ -87,6 +90,7 @@ int fpi_tau_from_counts(fp_ctx* ctx, const int32_t* cell_start, float tau_ref_n,
 {
     tau_kernel<<<fp_div_up(ctx->ncell, 256), 256, 0, st>>>(cell_start, ctx->ncell, tau_ref_n, ctx->p.tau, tau_cell);
     FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 1);
     return FP_OK;
 }
 
@@ -107,11 +111,16 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
         return fp_fail(ctx, FP_ERR_ARG, "fp_step: null particle pointer");
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    ctx->t_in_step = ctx->t_ev != nullptr && ctx->t_step < ctx->t_max;
+    struct step_guard { fp_ctx* c; ~step_guard() { if (c->t_in_step) { c->t_in_step = false; c->t_step += 1; } } } guard{ctx};
+    fp_mark(ctx, 0, st);
     // a0 + a1 (+ cell keys of the streamed positions)
     if ((rc = fpi_stream_walls(ctx, np, x_a, y_a, vx_a, vy_a, vz_a, pid_a, step, ctx->key_b, st)) != FP_OK) return rc;
-    // a2
+    fp_mark(ctx, 1, st);
+    // a2 (records mark 2 between the key sort and the payload gather)
     if ((rc = fpi_sort_with_keys(ctx, np, ctx->key_b, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b,
                                  cell_start, nullptr, st)) != FP_OK) return rc;
+    fp_mark(ctx, 3, st);
     const float* tau_use = nullptr;
     if (tau_mode == 1) {
         if ((rc = fpi_tau_from_counts(ctx, cell_start, tau_ref_n, tau_cell, st)) != FP_OK) return rc;
@@ -121,12 +130,57 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
     const int32_t mode = closure == 0 ? 1 : 0;
     const int32_t stride = mode ? 29 : 13;
     if ((rc = fp_cell_moments(ctx, np, vx_b, vy_b, vz_b, cell_start, mode, mom, stream)) != FP_OK) return rc;
+    fp_mark(ctx, 4, st);
     // a4 | a5
     if (closure == 0) rc = fp_closure_exact(ctx, mom, tau_use, coef, flags, nullptr, stream);
     else              rc = fp_closure_mlp(ctx, mom, stride, tau_use, h_mlp, relax_w, coef, flags, stream);
     if (rc != FP_OK) return rc;
+    fp_mark(ctx, 5, st);
     // a6
-    return fp_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, stream);
+    rc = fp_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, stream);
+    fp_mark(ctx, 6, st);
+    return rc;
+}
+
+extern "C" uint64_t fp_launch_count(const fp_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+static void fp_timing_free(fp_ctx* c)
+{
+    if (c->t_ev) {
+        for (size_t i = 0; i < (size_t)c->t_max * (FP_NSTAGES + 1); ++i) if (c->t_ev[i]) cudaEventDestroy(c->t_ev[i]);
+        delete[] c->t_ev;
+    }
+    c->t_ev = nullptr; c->t_max = 0; c->t_step = 0; c->t_in_step = false;
+}
+
+extern "C" int fp_timing_enable(fp_ctx* ctx, int32_t max_steps)
+{
+    if (!ctx || max_steps < 0 || max_steps > 65536) return FP_ERR_ARG;
+    fp_timing_free(ctx);
+    if (max_steps == 0) return FP_OK;
+    const size_t n = (size_t)max_steps * (FP_NSTAGES + 1);
+    ctx->t_ev = new (std::nothrow) cudaEvent_t[n]();
+    if (!ctx->t_ev) return fp_fail(ctx, FP_ERR_STATE, "fp_timing_enable: out of memory");
+    ctx->t_max = max_steps;
+    for (size_t i = 0; i < n; ++i) FP_CUDA_OK(ctx, cudaEventCreate(&ctx->t_ev[i]));
+    return FP_OK;
+}
+
+extern "C" int fp_timing_read(fp_ctx* ctx, float* h_ms, int32_t* h_nsteps)
+{
+    if (!ctx || !h_ms || !h_nsteps) return FP_ERR_ARG;
+    *h_nsteps = 0;
+    if (!ctx->t_ev) return fp_fail(ctx, FP_ERR_STATE, "fp_timing_read: timing is not enabled");
+    const int n = ctx->t_step;
+    if (n > 0) FP_CUDA_OK(ctx, cudaEventSynchronize(ctx->t_ev[(size_t)(n - 1) * (FP_NSTAGES + 1) + FP_NSTAGES]));
+    for (int s = 0; s < n; ++s)
+        for (int k = 0; k < FP_NSTAGES; ++k) {
+            const cudaEvent_t* e = ctx->t_ev + (size_t)s * (FP_NSTAGES + 1);
+            FP_CUDA_OK(ctx, cudaEventElapsedTime(&h_ms[s * FP_NSTAGES + k], e[k], e[k + 1]));
+        }
+    *h_nsteps = n;
+    ctx->t_step = 0;
+    return FP_OK;
 }
 
 static int fp_host_stage_alloc(fp_ctx* c)

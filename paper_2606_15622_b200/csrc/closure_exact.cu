@@ -211,5 +211,6 @@ extern "C" int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float
     closure_exact_kernel<<<blocks, CE_THREADS, 0, (cudaStream_t)stream>>>(mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
                                                                          ctx->p.min_count, ncell, coef, flags, kappa_est);
     FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 1);
     return FP_OK;
 }

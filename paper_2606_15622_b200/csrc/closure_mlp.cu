@@ -233,5 +233,6 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
         return fp_fail(ctx, FP_ERR_UNSUPPORTED, "fp_closure_mlp: hidden width > 512 is not supported");
     }
     FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 2);
     return FP_OK;
 }

@@ -51,8 +51,19 @@ struct fp_ctx {
     int32_t  *hs_cell_start = nullptr;
     bool      hs_ready = false;
     fp_mlp_dev mlp;
+    // measurement hooks
+    uint64_t  launches = 0;
+    cudaEvent_t* t_ev = nullptr;     // [t_max * (FP_NSTAGES + 1)]
+    int32_t   t_max = 0, t_step = 0;
+    bool      t_in_step = false;
     char      err[512];
 };
+
+// record the stage-boundary event `mark` (0..FP_NSTAGES) of the step being timed, if any
+static inline void fp_mark(fp_ctx* ctx, int mark, cudaStream_t st)
+{
+    if (ctx->t_in_step) cudaEventRecord(ctx->t_ev[(size_t)ctx->t_step * (FP_NSTAGES + 1) + mark], st);
+}
 
 static inline int fp_fail(fp_ctx* ctx, int code, const char* msg)
 {
@@ -71,6 +82,7 @@ static inline int fp_fail(fp_ctx* ctx, int code, const char* msg)
     } while (0)
 
 #define FP_LAUNCH_OK(ctx) FP_CUDA_OK(ctx, cudaGetLastError())
+#define FP_COUNT(ctx, n) ((ctx)->launches += (n))
 
 static inline int fp_div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 

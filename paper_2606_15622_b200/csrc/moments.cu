@@ -147,5 +147,6 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     else if (ppc >= 48.0)  launch_moments<8>(ctx, vx, vy, vz, cell_start, mode, mom, st);
     else                   launch_moments<4>(ctx, vx, vy, vz, cell_start, mode, mom, st);
     FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 1);
     return FP_OK;
 }

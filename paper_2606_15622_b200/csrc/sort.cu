@@ -180,6 +180,8 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
     if (np == 0) {
         zero_i32_kernel<<<fp_div_up(ncell + 1, 256), 256, 0, st>>>(cell_start, (int64_t)ncell + 1);
         FP_LAUNCH_OK(ctx);
+        FP_COUNT(ctx, 1);
+        fp_mark(ctx, 2, st);
         return FP_OK;
     }
     const int nblocks = fp_div_up(np, SORT_TILE);
@@ -201,6 +203,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
         else
             scatter_kernel<false><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, ctx->block_hist, ctx->bin_total, nblocks, shift, bins);
         FP_LAUNCH_OK(ctx);
+        FP_COUNT(ctx, 3);
         kin = kout; iin = iout;
         kout = (kout == ctx->key_a) ? ctx->key_b : ctx->key_a;
         iout = (iout == ctx->idx_a) ? ctx->idx_b : ctx->idx_a;
@@ -208,9 +211,11 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
     const int64_t cap = (int64_t)ctx->num_sms * 16;
     int64_t want = (np + 1 + 255) / 256;
     cell_start_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, kin, ncell, cell_start);
+    fp_mark(ctx, 2, st);
     want = (np + 255) / 256;
     gather_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, iin, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out, pid_out);
     FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 2);
     if (perm) FP_CUDA_OK(ctx, cudaMemcpyAsync(perm, iin, (size_t)np * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
     return FP_OK;
 }
@@ -235,6 +240,7 @@ extern "C" int fp_sort_by_cell(fp_ctx* ctx, int64_t np,
         const int64_t want = (np + 255) / 256;
         key_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, x, y, ctx->key_b, q.nx, q.ny, q.x0, q.y0, ctx->inv_dx, ctx->inv_dy);
         FP_LAUNCH_OK(ctx);
+        FP_COUNT(ctx, 1);
     }
     // keys live in key_b; the first pass writes key_a, so the ping-pong never overwrites its own input
     return fpi_sort_with_keys(ctx, np, ctx->key_b, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out,

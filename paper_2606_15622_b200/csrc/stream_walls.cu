@@ -136,6 +136,7 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
     if (keys_out) sw_kernel<true><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, keys_out, P);
     else          sw_kernel<false><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, nullptr, P);
     FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 1);
     return FP_OK;
 }
 

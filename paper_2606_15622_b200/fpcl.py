@@ -18,7 +18,10 @@ FP_OK, FP_ERR_ARG, FP_ERR_STATE, FP_ERR_CUDA, FP_ERR_UNSUPPORTED = 0, -1, -2, -3
 FLAG_EMPTY, FLAG_LOWCOUNT, FLAG_SINGULAR, FLAG_ILLCOND, FLAG_ALPHA, FLAG_SKIPPED, FLAG_NONFINITE = 1, 2, 4, 8, 16, 32, 64
 
 EXPORTS = ["fp_create", "fp_destroy", "fp_last_error", "fp_version", "fp_sort_by_cell", "fp_cell_moments",
-           "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host"]
+           "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host",
+           "fp_timing_enable", "fp_timing_read", "fp_launch_count"]
+NSTAGES = 6
+STAGE_NAMES = ["stream_walls", "sort_keys", "gather", "moments", "closure", "update"]
 
 
 class FpWall(C.Structure):
@@ -71,9 +74,13 @@ def load(path=None):
     lib.fp_stream_walls.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, u64, vp]
     lib.fp_step.argtypes = [vp, i64] + [vp] * 12 + [i32, C.POINTER(FpMlp), f32, i32, f32, vp, u64, vp, vp, vp, vp, vp]
     lib.fp_step_host.argtypes = [vp, i64] + [vp] * 6 + [i32, C.POINTER(FpMlp), f32, u64, vp, vp, vp, vp]
+    lib.fp_timing_enable.argtypes = [vp, i32]
+    lib.fp_timing_read.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32)]
+    lib.fp_launch_count.argtypes = [vp]
     for name in EXPORTS:
-        if name not in ("fp_last_error", "fp_version"):
+        if name not in ("fp_last_error", "fp_version", "fp_launch_count"):
             getattr(lib, name).restype = C.c_int
+    lib.fp_launch_count.restype = C.c_uint64
     if path is None:
         _lib = lib
     return lib
@@ -208,6 +215,22 @@ def fp_step_host(ctx, np_, h, closure, mlp, relax_w, step, h_coef=None, h_flags=
     _check(ctx, load().fp_step_host(ctx, np_, *args, closure, mp, relax_w, step, _hptr(h_coef, np.float32),
                                     _hptr(h_flags, np.uint32), _hptr(h_cell_start, np.int32), _stream()),
            "fp_step_host")
+
+
+def fp_timing_enable(ctx, max_steps):
+    _check(ctx, load().fp_timing_enable(ctx, max_steps), "fp_timing_enable")
+
+
+def fp_timing_read(ctx, max_steps):
+    """Returns an array [nsteps, NSTAGES] of stage durations in ms (see STAGE_NAMES)."""
+    buf = (C.c_float * (max_steps * NSTAGES))()
+    n = C.c_int32(0)
+    _check(ctx, load().fp_timing_read(ctx, buf, C.byref(n)), "fp_timing_read")
+    return np.frombuffer(buf, dtype=np.float32)[: n.value * NSTAGES].reshape(n.value, NSTAGES).copy()
+
+
+def fp_launch_count(ctx):
+    return int(load().fp_launch_count(ctx))
 
 
 # ---------------------------------------------------------------------------------------------- conveniences

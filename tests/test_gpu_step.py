@@ -4,7 +4,7 @@ bench.py times."""
 import numpy as np
 import pytest
 
-from parity_util import coef_ratio, moment_ratio, velocity_ratio
+from parity_util import abs_moments, coef_ratio, moment_ratio, velocity_ratio
 
 pytestmark = pytest.mark.gpu
 
@@ -164,8 +164,13 @@ def test_step_one(gpu, wl, orc, name, closure):
     assert np.array_equal(res["cell_start"], aux["cell_start"])
     assert np.array_equal(got["pid"], ref["pid"])
     assert np.array_equal(_bits(got["x"]), _bits(ref["x"])) and np.array_equal(_bits(got["y"]), _bits(ref["y"]))
-    # moments
-    rm = moment_ratio(res["mom"], aux["mom"])
+    # moments: 1e-6 where both sides saw bit-identical velocities; cells holding a re-emitted particle (whose fp32
+    # wall draw may differ from the oracle's fp64 one by up to 1e-6, R7) are compared at 1e-5
+    mid = orc.stream_walls(st, cfg, 3)
+    hit = (_bits(mid["vx"]) != _bits(st["vx"])) | (_bits(mid["vy"]) != _bits(st["vy"])) | (_bits(mid["vz"]) != _bits(st["vz"]))
+    touched = np.zeros(aux["mom"].shape[0], dtype=bool)
+    touched[orc.cell_index(mid["x"][hit], mid["y"][hit], cfg)] = True
+    rm = max(moment_ratio(res["mom"], aux["mom"], 1e-6, mask=~touched), moment_ratio(res["mom"], aux["mom"], 1e-5, mask=touched))
     assert rm <= 1.0
     theta = _theta(aux["mom"])
     tau = cfg["tau"] if tau_fn is None else tau_fn(aux["mom"][:, 0])
@@ -281,7 +286,7 @@ def test_full_size_cavity(gpu, wl, orc):
     d2 = gpu.to_device(s2)
     mom_g = ctx.cell_moments(d2["vx"], d2["vy"], d2["vz"], torch.from_numpy(cs).cuda(), 1).cpu().numpy()
     mom_o = orc.cell_moments(s2["vx"], s2["vy"], s2["vz"], cs, 1)
-    rm = moment_ratio(mom_g, mom_o)
+    rm = moment_ratio(mom_g, mom_o, absmom=abs_moments(s2["vx"], s2["vy"], s2["vz"], cs, mom_o))
     coef_o, fl_o, kappa = orc.closure_exact(mom_o, cfg["tau"], cfg["eps2_scale"], cfg["min_count"])
     coef_g, fl_g = ctx.closure_exact(torch.from_numpy(mom_o).cuda())
     ok = (fl_o & orc.FLAG_ILLCOND) == 0
