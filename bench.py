@@ -1,0 +1,407 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the cubic-FP closure hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl fpcl|reference] [--closure exact|mlp] [--small]
+
+One "step" = one fp_step (stream -> walls -> sort -> moment gather -> closure -> velocity update) over the
+BASELINE config-3 ensemble: 2D lid-driven cavity, 200x200 cells x 100 particles/cell = 4M particles, synthetic
+(seeded Maxwellian, 200 settling steps before timing so that cell counts are Poisson-like).  `value` is
+particle-steps/s with all inputs resident in HBM; `e2e` is the same metric through fp_step_host (pinned host
+buffers, H2D + D2H inside the timed region).  Multi-GPU (torchrun): every rank runs an independent replica with its
+own seed (weak scaling, no data-path collective -- DESIGN.md "Multi-GPU"); times are max-reduced over ranks.
+
+--impl reference times the CPU oracle (oracle/, plain C fp64, as it stands) on the host cores on a bounded sample
+of the same workload; it is a deliberately slow checker, not a competitor.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle_steps_per_s"
+UNIT = "particle-steps/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="fpcl", choices=["fpcl", "reference"])
+    ap.add_argument("--closure", default="exact", choices=["exact", "mlp"])
+    ap.add_argument("--settle", type=int, default=200, help="untimed steps that relax the initial uniform counts")
+    ap.add_argument("--small", action="store_true", help="64x64x100 cavity (debugging only; not a bench line)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the cold-L2 kernel table and the MLP variant")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def workload(args, seed):
+    from paper_2606_15622_b200 import workloads
+    n = 64 if args.small else 200
+    cfg, st = workloads.cavity(n=n, ppc=100, kn=0.5, seed=seed, shuffle=True)
+    name = "cavity Kn=0.5 %dx%d cells x 100 ppc = %d particles (BASELINE config 3%s)" % (
+        n, n, st["x"].shape[0], ", reduced" if args.small else "")
+    return cfg, st, name
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [v.strip() for v in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg, st, closure, mlp, max_seconds=25.0, max_steps=10):
+    """The oracle as it stands (one thread, fp64) stepping the same ensemble; returns (particle-steps/s, steps)."""
+    import oracle
+    oracle.build()
+    s = {k: v.copy() for k, v in st.items()}
+    n = s["x"].shape[0]
+    t0 = time.perf_counter()
+    done = 0
+    while done < max_steps:
+        s, _ = oracle.step(s, cfg, done, closure=closure, mlp=mlp)
+        done += 1
+        if time.perf_counter() - t0 > max_seconds:
+            break
+    dt = time.perf_counter() - t0
+    return n * done / dt, done, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config / metric / unit (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2606_15622_b200 import workloads
+    cfg, st, name = workload(args, seed=3)
+    mlp = workloads.xavier_mlp(n_scale=0.01, tau=cfg["tau"]) if args.closure == "mlp" else None
+    n = st["x"].shape[0]
+    # each "step" of this arm is one oracle step on a bounded sample: the first n_s particles' worth of cells
+    rows = 20 if not args.small else 8                      # 20 of 200 cell rows = 400k particles per step
+    ny = cfg["ny"]
+    keep = st["y"] < (rows / ny)
+    sub = {k: np.ascontiguousarray(v[keep]) for k, v in st.items()}
+    scfg = dict(cfg, ny=rows, max_particles=int(keep.sum()))
+    import oracle
+    oracle.build()
+    s = sub
+    for w in range(min(args.warmup, 1)):
+        s, _ = oracle.step(s, scfg, w, closure=args.closure, mlp=mlp)
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        s, _ = oracle.step(s, scfg, 100 + k, closure=args.closure, mlp=mlp)
+    dt = time.perf_counter() - t0
+    val = s["x"].shape[0] * args.steps / dt
+    sample = "%d oracle steps on a %dx%d-cell slab of the cavity (%d particles), 1 thread" % (
+        args.steps, cfg["nx"], rows, s["x"].shape[0])
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "closure": args.closure, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def algorithmic_bytes(np_, ncell):
+    """Algorithmic HBM bytes per launch."""
+    return {
+        "stream_walls": 28 * np_,                          # 16 r (x,y,vx,vy) + 8 w (x,y) + 4 w key
+        "moments_full": 12 * np_ + 236 * ncell,            # 12 B/particle + cell_start + 232 B record
+        "moments_lite": 12 * np_ + 108 * ncell,
+        "closure_exact": 272 * ncell,                      # 232 r + 36 w + 4 w flags
+        "closure_mlp": 144 * ncell,                        # 104 r + 36 w + 4 w
+        "update": 28 * np_ + (4 + 232 + 36 + 4) * ncell,   # 12 r + 4 r pid + 12 w; per cell start, record, coef, flags
+        "update_lite": 28 * np_ + (4 + 104 + 36 + 4) * ncell,
+        "gather": 52 * np_,                                # 4 r perm + 24 r + 24 w
+        "sort_keys": 36 * np_,                             # 2 passes x (4+4 r hist+scatter keys) + idx r/w
+    }
+
+
+def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
+    """Stand-alone launches of the judged kernels with an L2 flush (256 MB write) before each timed launch."""
+    np_ = state["x"].numel()
+    ncell = ctx.ncell
+    ab = algorithmic_bytes(np_, ncell)
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
+    cs = out["cell_start"]
+    mom_full = torch.empty((ncell, 29), dtype=torch.float64, device="cuda")
+    mom_lite = torch.empty((ncell, 13), dtype=torch.float64, device="cuda")
+    coef = torch.zeros((ncell, 9), dtype=torch.float32, device="cuda")
+    flags = torch.zeros(ncell, dtype=torch.int32, device="cuda")
+    v = [state[k].clone() for k in ("vx", "vy", "vz")]
+    ctx.cell_moments(v[0], v[1], v[2], cs, 1, out=mom_full)
+    ctx.cell_moments(v[0], v[1], v[2], cs, 0, out=mom_lite)
+    fpcl.fp_closure_exact(ctx.h, mom_full, None, coef, flags)
+
+    def timed(fn, key):
+        ts = []
+        for r in range(reps + 3):
+            flush.fill_(float(r))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn(r)
+            e1.record()
+            e1.synchronize()
+            if r >= 3:
+                ts.append(e0.elapsed_time(e1))
+        ms = float(np.median(ts))
+        gbs = ab[key] / (ms * 1e-3) / 1e9
+        return {"ms": ms, "best_ms": float(min(ts)), "GBps": gbs, "frac_of_hbm_peak": gbs / hbm_peak,
+                "algorithmic_bytes": ab[key]}
+
+    res = {}
+    res["moments_full"] = timed(lambda r: ctx.cell_moments(v[0], v[1], v[2], cs, 1, out=mom_full), "moments_full")
+    res["moments_lite"] = timed(lambda r: ctx.cell_moments(v[0], v[1], v[2], cs, 0, out=mom_lite), "moments_lite")
+    res["closure_exact"] = timed(lambda r: fpcl.fp_closure_exact(ctx.h, mom_full, None, coef, flags), "closure_exact")
+    res["closure_exact"]["cells_per_s"] = ncell / (res["closure_exact"]["ms"] * 1e-3)
+    if mlp_dev is not None:
+        res["closure_mlp"] = timed(lambda r: fpcl.fp_closure_mlp(ctx.h, mom_lite, 13, None, mlp_dev, 1.0, coef, flags),
+                                   "closure_mlp")
+        res["closure_mlp"]["cells_per_s"] = ncell / (res["closure_mlp"]["ms"] * 1e-3)
+    fpcl.fp_closure_exact(ctx.h, mom_full, None, coef, flags)
+    # the update rewrites velocities in place: each timed launch advances the same ensemble one collision step
+    ts = []
+    for r in range(reps + 3):
+        ctx.cell_moments(v[0], v[1], v[2], cs, 1, out=mom_full)      # moments of the current velocities (untimed)
+        flush.fill_(float(r))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.velocity_update(v[0], v[1], v[2], state["pid"], cs, mom_full, coef, 1000 + r, flags)
+        e1.record()
+        e1.synchronize()
+        if r >= 3:
+            ts.append(e0.elapsed_time(e1))
+    ms = float(np.median(ts))
+    gbs = ab["update"] / (ms * 1e-3) / 1e9
+    res["update"] = {"ms": ms, "best_ms": float(min(ts)), "GBps": gbs, "frac_of_hbm_peak": gbs / hbm_peak,
+                     "algorithmic_bytes": ab["update"], "particles_per_s": np_ / (ms * 1e-3)}
+    res["moments_full"]["particles_per_s"] = np_ / (res["moments_full"]["ms"] * 1e-3)
+    return res
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    import torch.distributed as dist
+    from paper_2606_15622_b200 import fpcl, workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm_peak, peak_src = peaks()
+    closure = 0 if args.closure == "exact" else 1
+
+    # independent replica per rank: same shape, different seed (weak scaling)
+    cfg, st, wname = workload(args, seed=3 + rank)
+    np_ = st["x"].shape[0]
+    ncell = cfg["nx"] * cfg["ny"]
+    mlp_host = workloads.xavier_mlp(n_scale=0.01, tau=cfg["tau"])
+    mlp_dev = fpcl.Mlp(mlp_host)
+    ctx = fpcl.Context(cfg)
+    a = fpcl.to_device(st)
+    b = {k: torch.empty_like(v) for k, v in a.items()}
+    out = ctx.alloc_step_outputs(closure)
+    step_no = 0
+    for _ in range(args.settle):
+        ctx.step(a, b, step_no, out, closure=closure, mlp=mlp_dev if closure else None)
+        a, b = b, a
+        step_no += 1
+    torch.cuda.synchronize()
+    settled = fpcl.to_host(a)                     # host copy of the settled ensemble: e2e and oracle input
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- timed region: K fp_step calls, device-resident
+    for _ in range(args.warmup):
+        ctx.step(a, b, step_no, out, closure=closure, mlp=mlp_dev if closure else None)
+        a, b = b, a
+        step_no += 1
+    fpcl.fp_timing_enable(ctx.h, args.steps)
+    l0 = fpcl.fp_launch_count(ctx.h)
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ctx.step(a, b, step_no, out, closure=closure, mlp=mlp_dev if closure else None)
+        a, b = b, a
+        step_no += 1
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    launches = fpcl.fp_launch_count(ctx.h) - l0
+    stage_ms = fpcl.fp_timing_read(ctx.h, args.steps)
+    fpcl.fp_timing_enable(ctx.h, 0)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    value = world * np_ * args.steps / (ms_total * 1e-3)
+    flags_host = out["flags"].cpu().numpy().view(np.uint32)
+
+    # ---- end to end through fp_step_host: pinned host buffers, H2D + D2H inside the timed region
+    pinned = {k: torch.from_numpy(v.view(np.int32) if k == "pid" else v).pin_memory() for k, v in settled.items()}
+    hc = torch.empty((ncell, 9), dtype=torch.float32).pin_memory()
+    hf = torch.empty(ncell, dtype=torch.int32).pin_memory()
+    hs = torch.empty(ncell + 1, dtype=torch.int32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    for w in range(2):
+        ctx.step_host(pinned, 10_000 + w, closure=closure, mlp=mlp_dev if closure else None, h_coef=hc, h_flags=hf,
+                      h_cell_start=hs)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(e2e_steps):
+        ctx.step_host(pinned, 20_000 + k, closure=closure, mlp=mlp_dev if closure else None, h_coef=hc, h_flags=hf,
+                      h_cell_start=hs)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * np_ * e2e_steps / float(t.item())
+    h2d = 24 * np_
+    d2h = 24 * np_ + ncell * (36 + 4) + (ncell + 1) * 4
+
+    # ---- per-stage times inside the timed region (CUDA events recorded by the library on the launch stream)
+    ab = algorithmic_bytes(np_, ncell)
+    med = np.median(stage_ms, axis=0) if stage_ms.shape[0] else np.zeros(fpcl.NSTAGES)
+    stage_bytes = [ab["stream_walls"], ab["sort_keys"], ab["gather"], ab["moments_full" if closure == 0 else "moments_lite"],
+                   ab["closure_exact" if closure == 0 else "closure_mlp"], ab["update" if closure == 0 else "update_lite"]]
+    stages = {}
+    for k, nme in enumerate(fpcl.STAGE_NAMES):
+        gbs = stage_bytes[k] / (med[k] * 1e-3) / 1e9 if med[k] > 0 else 0.0
+        stages[nme] = {"ms": float(med[k]), "share": float(med[k] / med.sum()) if med.sum() > 0 else 0.0,
+                       "GBps_algorithmic": gbs, "frac_of_hbm_peak": gbs / hbm_peak}
+    # dominant single kernel of the step (sort_keys is six launches; the others are one kernel each)
+    single = {n: stages[n] for n in ("stream_walls", "gather", "moments", "closure", "update")}
+    dom = max(single, key=lambda n: single[n]["ms"])
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": single[dom]["GBps_algorithmic"], "peak": hbm_peak,
+                "unit": "GB/s", "frac": single[dom]["frac_of_hbm_peak"], "traffic": None,
+                "peak_source": peak_src, "timing": "CUDA events inside fp_step, median over the timed steps (L2-warm)"}
+
+    extras = {}
+    if rank == 0 and not args.no_extras:
+        extras["kernels_cold_l2"] = cold_kernel_table(fpcl, torch, ctx, a, out, mlp_dev, hbm_peak)
+        # the surrogate variant of the whole step (Algorithm 2), short run
+        out2 = ctx.alloc_step_outputs(1)
+        a2 = {k: v.clone() for k, v in a.items()}
+        b2 = {k: torch.empty_like(v) for k, v in a.items()}
+        for w in range(3):
+            ctx.step(a2, b2, 50_000 + w, out2, closure=1, mlp=mlp_dev); a2, b2 = b2, a2
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        nrep = min(args.steps, 20)
+        for w in range(nrep):
+            ctx.step(a2, b2, 60_000 + w, out2, closure=1, mlp=mlp_dev); a2, b2 = b2, a2
+        f1.record(); f1.synchronize()
+        extras["step_with_mlp_closure"] = {"ms_per_step": f0.elapsed_time(f1) / nrep,
+                                           "particle_steps_per_s": np_ * nrep / (f0.elapsed_time(f1) * 1e-3)}
+
+    cpu_baseline = None
+    if rank == 0 and not args.no_cpu_baseline:
+        v, done, dt = oracle_sample(cfg, settled, args.closure, mlp_host if closure else None)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                        "sample": "%d full fp_step(s) of the same %d-particle ensemble by oracle/ (%.1f s)" % (done, np_, dt)}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": wname, "closure": args.closure, "particles_per_gpu": np_, "cells": ncell,
+                           "settle_steps": args.settle, "parallelism": "replicas x%d (independent seeds)" % world,
+                           "l2": "working set (two SoA copies + sort scratch = %d MB) exceeds the 126 MB L2; no "
+                                 "explicit flush between steps" % ((48 * np_ + 16 * np_) // (1 << 20))},
+                "closure_cells_per_s": ncell / (stages["closure"]["ms"] * 1e-3) if stages["closure"]["ms"] > 0 else None,
+                "clocks": clocks,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "steps": e2e_steps, "api": "fp_step_host (pinned host buffers)"},
+                "gpu_launches": int(launches),
+                "roofline": roofline, "stages": stages, "cpu_baseline": cpu_baseline,
+                "flags_nonzero_cells": int((flags_host != 0).sum())}
+        line.update(extras)
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
