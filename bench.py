@@ -397,7 +397,7 @@ def main():
                 "roofline": roofline, "stages": stages, "cpu_baseline": cpu_baseline,
                 "flags_nonzero_cells": int((flags_host != 0).sum())}
         line.update(extras)
-        print(json.dumps(line))
+        print(json.dumps(line, default=float))
     ctx.close()
     if world > 1:
         dist.destroy_process_group()
