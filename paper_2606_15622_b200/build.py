@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJDIR = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libfpcl.so")
-SOURCES = ["api.cu", "stream_walls.cu", "sort.cu", "moments.cu", "closure_exact.cu", "closure_mlp.cu", "update.cu"]
+SOURCES = ["api.cu", "tiles.cu", "stream_walls.cu", "sort.cu", "moments.cu", "closure_exact.cu", "closure_mlp.cu", "update.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
          "-I", INCLUDE]
@@ -30,7 +30,7 @@ def _newer(target, deps):
 
 def build(force=False, verbose=False):
     os.makedirs(OBJDIR, exist_ok=True)
-    headers = [os.path.join(CSRC, "common.cuh"), os.path.join(INCLUDE, "fpcl.h"), os.path.abspath(__file__)]
+    headers = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "tiles.cuh"), os.path.join(INCLUDE, "fpcl.h"), os.path.abspath(__file__)]
     jobs = []
     objs = []
     for s in SOURCES:

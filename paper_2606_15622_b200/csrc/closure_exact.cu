@@ -8,13 +8,13 @@
 //                          = -(4/(3 tau)) h_i + eps2 (3 g_i - 3 theta h_i - 2 P_ik h_k)
 // assembled in scaled variables (velocity unit sqrt(theta), time unit tau; R3-a), so all entries are O(1).
 //
-// Mapping: 16 lanes per cell, lane r < 9 owns row r (9 matrix entries + rhs in registers, fp64).  The system never
-// touches HBM: 232 B/cell in, 40 B/cell out.  Pivot search = 4-step butterfly arg-max; the pivot row is
-// broadcast by shuffles; rows are never swapped physically (a row remembers the step it was used as pivot).
+// Mapping: one thread per cell, fp64.  The block first stages its cells' records with coalesced loads into shared
+// memory (stride 29 doubles is bank-conflict free), each thread scales its record in registers, writes its augmented
+// 9x10 system to shared memory as [entry][thread] (conflict free, dynamic row index = free pivoting without register
+// selects) and eliminates in place.  The system never touches HBM: 232 B/cell in, 40 B/cell out.
 #include "common.cuh"
 
-#define CE_THREADS 128
-#define CE_G 16
+#define CE_TPB 64
 
 __host__ __device__ constexpr int ce_s2(int i, int j) { return i <= j ? i * (5 - i) / 2 + j : j * (5 - j) / 2 + i; }
 __host__ __device__ constexpr int ce_s3(int i, int j, int k)
@@ -67,31 +67,48 @@ __device__ __forceinline__ void ce_build_row(const ce_scaled& m, double (&a)[10]
     }
 }
 
-__global__ void __launch_bounds__(CE_THREADS)
+__global__ void __launch_bounds__(CE_TPB)
 closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ tau_cell, float tau_scalar,
                      float eps2_scale, int32_t min_count, int32_t ncell, float* __restrict__ coef,
                      uint32_t* __restrict__ flags, double* __restrict__ kappa_est)
 {
-    const int lane = threadIdx.x & 31;
-    const int gl = lane & (CE_G - 1);
-    const int gbase = lane & ~(CE_G - 1);
-    const int64_t cell = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / CE_G;
-    const bool have = cell < ncell;
-    const double* rec = mom + (size_t)(have ? cell : 0) * 29;
+    extern __shared__ double ce_sm[];
+    double* recs = ce_sm;                        // [CE_TPB * 29] staged records
+    double* As = ce_sm + CE_TPB * 29;            // [90][CE_TPB] augmented systems
+    const int tid = threadIdx.x;
+    const int64_t cell0 = (int64_t)blockIdx.x * CE_TPB;
+    const int ncb = (int)min((int64_t)CE_TPB, (int64_t)ncell - cell0);
+    for (int e = tid; e < ncb * 29; e += CE_TPB) recs[e] = mom[(size_t)cell0 * 29 + e];
+    __syncthreads();
+    if (tid >= ncb) return;
+    const int64_t cell = cell0 + tid;
+    const double* rec = recs + tid * 29;
     const double n = rec[0];
-    const double tau = (double)(tau_cell ? tau_cell[have ? cell : 0] : tau_scalar);
-    double theta = (rec[4] + rec[7] + rec[9]) / 3.0;
+    const double tau = (double)(tau_cell ? tau_cell[cell] : tau_scalar);
+    const double theta = (rec[4] + rec[7] + rec[9]) / 3.0;
     const bool theta_ok = (theta > 0.0) && isfinite(theta);
-    const double th = theta_ok ? theta : 1.0;            // keep the arithmetic finite on cells that fall back
-    ce_scaled m;
+    float* out = coef + (size_t)cell * 9;
+    // ---- policy for cells that are not solved (R3-c)
+    if (!(n > 0.0) || n < (double)min_count || !theta_ok) {
+        const bool empty = !(n > 0.0);
+        const float d = empty ? 0.0f : (float)(-1.0 / tau);
+        out[0] = d; out[1] = 0.f; out[2] = 0.f; out[3] = d; out[4] = 0.f; out[5] = d; out[6] = 0.f; out[7] = 0.f; out[8] = 0.f;
+        flags[cell] = empty ? FP_FLAG_EMPTY : (n < (double)min_count ? FP_FLAG_LOWCOUNT : FP_FLAG_SINGULAR);
+        if (kappa_est) kappa_est[cell] = 0.0;
+        return;
+    }
+#define CE_A(i, j) As[((i) * 10 + (j)) * CE_TPB + tid]
+    double anorm = 0.0, bmax = 0.0;
     {
-        const double s1 = sqrt(th), s2 = th, s3 = th * s1, s4 = th * th, s5 = s4 * s1;
+        ce_scaled m;
+        const double it = 1.0 / theta, s1 = sqrt(theta);
+        const double i2 = it, i3 = it / s1, i4 = it * it, i5 = i4 / s1;
 #pragma unroll
-        for (int k = 0; k < 6; ++k) { m.P[k] = rec[4 + k] / s2; m.Fij[k] = rec[20 + k] / s4; }
+        for (int k = 0; k < 6; ++k) { m.P[k] = rec[4 + k] * i2; m.Fij[k] = rec[20 + k] * i4; }
 #pragma unroll
-        for (int k = 0; k < 10; ++k) m.t[k] = rec[10 + k] / s3;
+        for (int k = 0; k < 10; ++k) m.t[k] = rec[10 + k] * i3;
 #pragma unroll
-        for (int k = 0; k < 3; ++k) m.g[k] = rec[26 + k] / s5;
+        for (int k = 0; k < 3; ++k) m.g[k] = rec[26 + k] * i5;
         m.F = 0.0;
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
@@ -103,101 +120,88 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
         // eps2_hat = eps2 tau theta = eps2_scale |det(P/theta - I)|   (R2-e)
         const double a = m.P[0] - 1.0, b = m.P[1], c = m.P[2], d = m.P[3] - 1.0, e = m.P[4], f = m.P[5] - 1.0;
         m.e2 = (double)eps2_scale * fabs(a * (d * f - e * e) - b * (b * f - e * c) + c * (b * e - d * c));
+        double row[10];
+#define CE_ROW(R)                                                                         \
+        ce_build_row<R>(m, row);                                                          \
+        { double rs = 0.0;                                                                \
+          _Pragma("unroll") for (int j = 0; j < 10; ++j) CE_A(R, j) = row[j];             \
+          _Pragma("unroll") for (int j = 0; j < 9; ++j) rs += fabs(row[j]);               \
+          anorm = fmax(anorm, rs); bmax = fmax(bmax, fabs(row[9])); }
+        CE_ROW(0) CE_ROW(1) CE_ROW(2) CE_ROW(3) CE_ROW(4) CE_ROW(5) CE_ROW(6) CE_ROW(7) CE_ROW(8)
+#undef CE_ROW
     }
-    double a[10];
-    switch (gl) {
-        case 0: ce_build_row<0>(m, a); break;
-        case 1: ce_build_row<1>(m, a); break;
-        case 2: ce_build_row<2>(m, a); break;
-        case 3: ce_build_row<3>(m, a); break;
-        case 4: ce_build_row<4>(m, a); break;
-        case 5: ce_build_row<5>(m, a); break;
-        case 6: ce_build_row<6>(m, a); break;
-        case 7: ce_build_row<7>(m, a); break;
-        case 8: ce_build_row<8>(m, a); break;
-        default:
+    // ---- Gaussian elimination with partial pivoting; perm[k] = storage row used as the k-th pivot row
+    int perm[9];
 #pragma unroll
-            for (int k = 0; k < 10; ++k) a[k] = 0.0;
-    }
-    __syncwarp();
-    // norms for the condition estimate: ||A||_inf and ||b||_inf
-    double rowsum = 0.0;
-#pragma unroll
-    for (int k = 0; k < 9; ++k) rowsum += fabs(a[k]);
-    double bmax = fabs(a[9]);
-#pragma unroll
-    for (int d = CE_G / 2; d >= 1; d >>= 1) {
-        rowsum = fmax(rowsum, fpd_shfl_xor(rowsum, d));
-        bmax = fmax(bmax, fpd_shfl_xor(bmax, d));
-    }
-    // ---- elimination with partial pivoting, row per lane
-    bool used = gl >= 9;
-    int piv_lane[9];
+    for (int k = 0; k < 9; ++k) perm[k] = k;
     double minpiv = INFINITY, maxpiv = 0.0;
+    uint32_t used = 0;                            // bit r set: storage row r already served as a pivot row
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
-        double cand = used ? -1.0 : fabs(a[k]);
-        if (!(cand >= -1.0)) cand = 0.0;                  // NaN
-        double best = cand;
-        int bl = gl;
+        // pivot search over the rows not yet used, in the order the swapped matrix of the textbook algorithm
+        // would hold them: position k first (the row displaced there by earlier swaps), then k+1..8
+        double best = -1.0;
+        int pr = 0, ppos = k;
 #pragma unroll
-        for (int d = CE_G / 2; d >= 1; d >>= 1) {
-            const double ob = fpd_shfl_xor(best, d);
-            const int ol = __shfl_xor_sync(0xffffffffu, bl, d);
-            if (ob > best || (ob == best && ol < bl)) { best = ob; bl = ol; }
+        for (int pos = k; pos < 9; ++pos) {
+            const int r = perm[pos];
+            double v = fabs(CE_A(r, k));
+            if (!(v >= 0.0)) v = 0.0;
+            if (v > best) { best = v; pr = r; ppos = pos; }
         }
-        piv_lane[k] = bl;
+        // swap positions k and ppos (bookkeeping only)
+#pragma unroll
+        for (int pos = k; pos < 9; ++pos) if (pos == ppos) { perm[pos] = perm[k]; }
+        perm[k] = pr;
+        used |= 1u << pr;
         minpiv = fmin(minpiv, best);
         maxpiv = fmax(maxpiv, best);
-        double pr[10];
+        double prow[10];
 #pragma unroll
-        for (int j = k; j < 10; ++j) pr[j] = fpd_shfl(a[j], gbase + bl);
-        if (gl == bl) used = true;
-        else if (!used) {
-            const double f = a[k] / pr[k];
+        for (int j = k; j < 10; ++j) prow[j] = CE_A(pr, j);
+        const double inv = 1.0 / prow[k];
 #pragma unroll
-            for (int j = k + 1; j < 10; ++j) a[j] -= f * pr[j];
-            a[k] = 0.0;
+        for (int r = 0; r < 9; ++r) {
+            if (!((used >> r) & 1u)) {
+                const double f = CE_A(r, k) * inv;
+#pragma unroll
+                for (int j = k + 1; j < 10; ++j) CE_A(r, j) -= f * prow[j];
+            }
         }
     }
-    // ---- back substitution: the row used at step k yields y[k]
+    // ---- back substitution
     double y[9];
 #pragma unroll
     for (int k = 8; k >= 0; --k) {
-        double s = a[9];
+        const int r = perm[k];
+        double s = CE_A(r, 9);
 #pragma unroll
-        for (int j = k + 1; j < 9; ++j) s -= a[j] * y[j];
-        s /= a[k];
-        y[k] = fpd_shfl(s, gbase + piv_lane[k]);
+        for (int j = k + 1; j < 9; ++j) s -= CE_A(r, j) * y[j];
+        y[k] = s / CE_A(r, k);
     }
+#undef CE_A
     bool finite = true;
     double ymax = 0.0;
 #pragma unroll
     for (int k = 0; k < 9; ++k) { finite = finite && isfinite(y[k]); ymax = fmax(ymax, fabs(y[k])); }
-    // ---- policy (R3-c) and output
     uint32_t flag = 0;
-    double out = 0.0;
-    const bool langevin_row = (gl == 0 || gl == 3 || gl == 5);
-    const double lang = langevin_row ? -1.0 / tau : 0.0;
     double kap = 0.0;
-    if (!(n > 0.0)) { flag = FP_FLAG_EMPTY; out = 0.0; }
-    else if (n < (double)min_count) { flag = FP_FLAG_LOWCOUNT; out = lang; }
-    else if (!theta_ok) { flag = FP_FLAG_SINGULAR; out = lang; }
-    else if (!(minpiv >= 1e-14) || !finite) { flag = FP_FLAG_SINGULAR; out = lang; }
-    else {
-        const double k1 = bmax > 0.0 ? rowsum * ymax / bmax : 0.0;
-        const double k2 = maxpiv / minpiv;
-        kap = fmax(k1, k2);
+    if (!(minpiv >= 1e-14) || !finite) {
+        const float d = (float)(-1.0 / tau);
+        out[0] = d; out[1] = 0.f; out[2] = 0.f; out[3] = d; out[4] = 0.f; out[5] = d; out[6] = 0.f; out[7] = 0.f; out[8] = 0.f;
+        flag = FP_FLAG_SINGULAR;
+    } else {
+        const double k1 = bmax > 0.0 ? anorm * ymax / bmax : 0.0;
+        kap = fmax(k1, maxpiv / minpiv);
         if (!(kap < 1e8)) flag = FP_FLAG_ILLCOND;
-        double yk = 0.0;
+        const double ic = 1.0 / tau, ig = 1.0 / (tau * sqrt(theta));
 #pragma unroll
-        for (int k = 0; k < 9; ++k) if (gl == k) yk = y[k];
-        out = (gl < 6) ? yk / tau : yk / (tau * sqrt(theta));
+        for (int k = 0; k < 6; ++k) out[k] = (float)(y[k] * ic);
+#pragma unroll
+        for (int k = 6; k < 9; ++k) out[k] = (float)(y[k] * ig);
     }
-    if (have) {
-        if (gl < 9) coef[(size_t)cell * 9 + gl] = (float)out;
-        if (gl == 0) { flags[cell] = flag; if (kappa_est) kappa_est[cell] = kap; }
-    }
+    flags[cell] = flag;
+    if (kappa_est) kappa_est[cell] = kap;
 }
 
 extern "C" int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell, float* coef,
@@ -206,10 +210,15 @@ extern "C" int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float
     if (!ctx) return FP_ERR_ARG;
     if (!mom_full || !coef || !flags) return fp_fail(ctx, FP_ERR_ARG, "fp_closure_exact: null pointer");
     const int32_t ncell = ctx->ncell;
-    const int cells_per_block = CE_THREADS / CE_G;
-    const int blocks = fp_div_up(ncell, cells_per_block);
-    closure_exact_kernel<<<blocks, CE_THREADS, 0, (cudaStream_t)stream>>>(mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
-                                                                         ctx->p.min_count, ncell, coef, flags, kappa_est);
+    const int blocks = fp_div_up(ncell, CE_TPB);
+    const size_t smem = (size_t)CE_TPB * (29 + 90) * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+        FP_CUDA_OK(ctx, cudaFuncSetAttribute(closure_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    closure_exact_kernel<<<blocks, CE_TPB, smem, (cudaStream_t)stream>>>(mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
+                                                                       ctx->p.min_count, ncell, coef, flags, kappa_est);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
     return FP_OK;

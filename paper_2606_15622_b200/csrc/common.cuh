@@ -42,6 +42,8 @@ struct fp_ctx {
     uint32_t *block_hist = nullptr;  // [bins][nblocks]
     uint32_t *bin_total = nullptr;   // [bins]
     size_t    block_hist_elems = 0;
+    int32_t  *tile_cell = nullptr;   // [max_particles / FPT_T + 2] first cell of each particle tile (tiles.cuh)
+    float    *cellc = nullptr;       // [ncell * 24] per-cell constants of the velocity update (update.cu)
     // fp_step_host staging (allocated lazily)
     float    *hs_f[2][5] = {{nullptr}};
     uint32_t *hs_pid[2] = {nullptr, nullptr};
