@@ -4,7 +4,7 @@
 #include <math.h>
 #include <new>
 
-#include "common.cuh"
+#include "tiles.cuh"
 
 static const char* k_version = "fpcl 0.1 (sm_100a)";
 
@@ -15,7 +15,7 @@ extern "C" const char* fp_last_error(const fp_ctx* ctx) { return ctx ? ctx->err 
 static void fp_free_all(fp_ctx* c)
 {
     cudaFree(c->key_a); cudaFree(c->key_b); cudaFree(c->idx_a); cudaFree(c->idx_b);
-    cudaFree(c->block_hist); cudaFree(c->bin_total); cudaFree(c->tile_cell); cudaFree(c->cellc);
+    cudaFree(c->block_hist); cudaFree(c->bin_total); cudaFree(c->cellc);
     for (int s = 0; s < 2; ++s) { for (int k = 0; k < 5; ++k) cudaFree(c->hs_f[s][k]); cudaFree(c->hs_pid[s]); }
     cudaFree(c->hs_mom); cudaFree(c->hs_coef); cudaFree(c->hs_flags); cudaFree(c->hs_cell_start);
     cudaFree(c->mlp.blob);
@@ -60,8 +60,7 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
               cudaMalloc((void**)&c->idx_a, n * 4) == cudaSuccess && cudaMalloc((void**)&c->idx_b, n * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->block_hist, c->block_hist_elems * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->bin_total, 512 * 4) == cudaSuccess &&
-              cudaMalloc((void**)&c->tile_cell, (n / 2048 + 2) * 4) == cudaSuccess &&
-              cudaMalloc((void**)&c->cellc, (size_t)c->ncell * 24 * 4) == cudaSuccess;
+              cudaMalloc((void**)&c->cellc, (size_t)c->ncell * 28 * 4) == cudaSuccess;
     if (!ok) { fp_free_all(c); delete c; cudaGetLastError(); return FP_ERR_CUDA; }
     *out = c;
     return FP_OK;
@@ -139,7 +138,7 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
     if (rc != FP_OK) return rc;
     fp_mark(ctx, 5, st);
     // a6
-    rc = fp_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, stream);
+    rc = fpi_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, st);
     fp_mark(ctx, 6, st);
     return rc;
 }

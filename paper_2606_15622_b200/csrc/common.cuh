@@ -42,8 +42,7 @@ struct fp_ctx {
     uint32_t *block_hist = nullptr;  // [bins][nblocks]
     uint32_t *bin_total = nullptr;   // [bins]
     size_t    block_hist_elems = 0;
-    int32_t  *tile_cell = nullptr;   // [max_particles / FPT_T + 2] first cell of each particle tile (tiles.cuh)
-    float    *cellc = nullptr;       // [ncell * 24] per-cell constants of the velocity update (update.cu)
+    float    *cellc = nullptr;       // [ncell * 28] per-cell constants of the velocity update (update.cu)
     // fp_step_host staging (allocated lazily)
     float    *hs_f[2][5] = {{nullptr}};
     uint32_t *hs_pid[2] = {nullptr, nullptr};
@@ -153,8 +152,10 @@ __device__ __forceinline__ double fpd_shfl(double v, int src)
 // Transposing ("multi-value") butterfly over a group of G lanes (G a power of two, groups aligned).
 // In:  v[0..NP) per lane (NP a power of two, NP >= G).  Out: v[0..NP/G) of lane L (L = lane index inside the
 // group) holds the group sum of original slots (NP/G)*L + i.  (NP - NP/G) 64-bit shuffles instead of NP*log2(G).
-template <int NP, int G>
-__device__ __forceinline__ void fpd_transpose_reduce(double (&v)[NP], int lane_in_group)
+__device__ __forceinline__ float fpd_shfl_xor(float v, int mask) { return __shfl_xor_sync(0xffffffffu, v, mask); }
+
+template <int NP, int G, typename T>
+__device__ __forceinline__ void fpd_transpose_reduce(T (&v)[NP], int lane_in_group)
 {
     static_assert((NP & (NP - 1)) == 0 && (G & (G - 1)) == 0 && NP >= G, "powers of two");
 #pragma unroll
@@ -163,8 +164,8 @@ __device__ __forceinline__ void fpd_transpose_reduce(double (&v)[NP], int lane_i
         const int h = n >> 1;
 #pragma unroll
         for (int i = 0; i < h; ++i) {
-            const double send = up ? v[i] : v[i + h];
-            const double keep = up ? v[i + h] : v[i];
+            const T send = up ? v[i] : v[i + h];
+            const T keep = up ? v[i + h] : v[i];
             v[i] = keep + fpd_shfl_xor(send, half);
         }
     }

@@ -2,20 +2,22 @@
 // (PAPER.md:124 moment definition, :215-216 M1-M5, :243 LITE, :181 plain 1/N mean; R0).
 //
 // HBM-bound by design: 12 B/particle read once + one record per cell written.
-// One CTA per particle tile (tiles.cuh): the tile's vx, vy, vz slices are staged in shared memory by three 1D bulk
-// asynchronous copies, then a group of G lanes (G = 4/8/16 by mean particles per cell) owns one cell, so a warp
-// works on 32/G cells at once and both passes over a cell read shared memory:
+// A group of G lanes (G = 4/8/16 by mean particles per cell) owns one cell, so a warp works on 32/G consecutive cells
+// at once.  Each warp stages the contiguous vx, vy, vz slices of its cells in its own shared-memory buffer with three
+// 1D bulk asynchronous copies (tiles.cuh) -- HBM is read once, coalesced, with no block-wide barrier and no
+// dependence between warps -- and both passes over a cell read shared memory:
 //   pass 1: S = sum (v - v_pivot) in fp32 about the cell's first particle (differences are thermal-sized, so fp32
 //           holds them to ~6e-8 of the thermal speed even at Mach 10), reduced across the group in fp64;
 //           U = v_pivot + S/N (fp64), m = S/N.
 //   pass 2: c = (v - v_pivot) - m in fp32, monomials and per-lane partial sums in fp32 (<= 64 terms per lane and
-//           chunk), converted to fp64 and reduced across the group with a transposing butterfly that leaves record
-//           slot k in the lane that stores it.
-// Cells larger than G*64 particles are processed chunk by chunk with fp64 accumulation between chunks.  A tile that
-// does not fit the staging buffer (a huge cell) or unaligned arrays run the same code on global pointers.
+//           chunk), combined across the group by a balanced fp32 tree (a transposing butterfly that leaves record
+//           slot k in the lane that stores it); chunks, the mean and the 1/N normalisation are fp64.
+// Cells larger than G*64 particles are processed chunk by chunk with fp64 accumulation between chunks.  A warp whose
+// cells do not fit its staging buffer (dense or huge cells), or unaligned arrays, run the same code on global pointers.
 #include "tiles.cuh"
 
 #define MOM_THREADS 128
+#define MOM_WARPS (MOM_THREADS / 32)
 #define MOM_CHUNK_PER_LANE 64
 
 // One cell per group of G lanes.  bx/by/bz may point to shared or global memory; particle p is at b?[p].
@@ -58,7 +60,7 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
         float F0 = 0.f, F1 = 0.f, F2 = 0.f, F3 = 0.f, F4 = 0.f, F5 = 0.f;
         float g0 = 0.f, g1 = 0.f, g2 = 0.f;
         const int32_t cend = min(n, c0 + G * MOM_CHUNK_PER_LANE);
-#pragma unroll 2
+#pragma unroll 4
         for (int32_t j = c0 + gl; j < cend; j += G) {
             const float cx = (bx[s + j] - px) - m0, cy = (by[s + j] - py) - m1, cz = (bz[s + j] - pz) - m2;
             const float xx = cx * cx, xy = cx * cy, xz = cx * cz, yy = cy * cy, yz = cy * cz, zz = cz * cz;
@@ -76,24 +78,23 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
                 g0 = fmaf(c2, cx, g0); g1 = fmaf(c2, cy, g1); g2 = fmaf(c2, cz, g2);      // h_i = <c^2 c_i>
             }
         }
-        double r[NP];
-        r[0] = r[1] = r[2] = r[3] = 0.0;
-        r[4] = (double)P0; r[5] = (double)P1; r[6] = (double)P2; r[7] = (double)P3; r[8] = (double)P4; r[9] = (double)P5;
+        float r[NP];
+        r[0] = r[1] = r[2] = r[3] = 0.f;
+        r[4] = P0; r[5] = P1; r[6] = P2; r[7] = P3; r[8] = P4; r[9] = P5;
         if (FULL) {
-            r[10] = (double)t0; r[11] = (double)t1; r[12] = (double)t2; r[13] = (double)t3; r[14] = (double)t4;
-            r[15] = (double)t5; r[16] = (double)t6; r[17] = (double)t7; r[18] = (double)t8; r[19] = (double)t9;
-            r[20] = (double)F0; r[21] = (double)F1; r[22] = (double)F2; r[23] = (double)F3; r[24] = (double)F4;
-            r[25] = (double)F5; r[26] = (double)g0; r[27] = (double)g1; r[28] = (double)g2;
+            r[10] = t0; r[11] = t1; r[12] = t2; r[13] = t3; r[14] = t4; r[15] = t5; r[16] = t6; r[17] = t7; r[18] = t8;
+            r[19] = t9; r[20] = F0; r[21] = F1; r[22] = F2; r[23] = F3; r[24] = F4; r[25] = F5; r[26] = g0; r[27] = g1;
+            r[28] = g2;
 #pragma unroll
-            for (int k = 29; k < NP; ++k) r[k] = 0.0;
+            for (int k = 29; k < NP; ++k) r[k] = 0.f;
         } else {
-            r[10] = (double)g0; r[11] = (double)g1; r[12] = (double)g2;
+            r[10] = g0; r[11] = g1; r[12] = g2;
 #pragma unroll
-            for (int k = 13; k < NP; ++k) r[k] = 0.0;
+            for (int k = 13; k < NP; ++k) r[k] = 0.f;
         }
-        fpd_transpose_reduce<NP, G>(r, gl);
+        fpd_transpose_reduce<NP, G, float>(r, gl);       // balanced fp32 tree over the group's partial sums
 #pragma unroll
-        for (int i = 0; i < PER; ++i) tot[i] += r[i];
+        for (int i = 0; i < PER; ++i) tot[i] += (double)r[i];
     }
     // lane gl holds record slots PER*gl .. PER*gl + PER - 1
     if (have) {
@@ -110,46 +111,52 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     }
 }
 
+// One warp = one chunk of 32/G consecutive cells, staged and processed independently of the other warps of the CTA.
 template <int G, bool FULL>
 __global__ void __launch_bounds__(MOM_THREADS)
-moments_tile_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
-                    const int32_t* __restrict__ cell_start, const int32_t* __restrict__ tile_cell, int32_t ncell,
-                    int64_t np, int32_t aligned, double* __restrict__ mom)
+moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
+                    const int32_t* __restrict__ cell_start, int32_t ncell, int64_t np, int32_t aligned,
+                    double* __restrict__ mom)
 {
     constexpr int NREC = FULL ? 29 : 13;
-    __shared__ __align__(16) float sx[FPT_CAP], sy[FPT_CAP], sz[FPT_CAP];
-    __shared__ __align__(8) uint64_t bar;
-    const fpt_tile t = fpt_tile_of_block(tile_cell, cell_start, ncell, np, aligned != 0);
-    if (t.c0 >= t.c1) return;
-    const float *bx = vx, *by = vy, *bz = vz;
-    if (t.staged) {
-        const uint32_t bytes = (uint32_t)t.nb * 4u;
-        if (threadIdx.x == 0 && bytes > 0) fpt_mbar_init(&bar, 1);
-        __syncthreads();
-        if (threadIdx.x == 0 && bytes > 0) {
-            fpt_mbar_expect_tx(&bar, 3u * bytes);
-            fpt_bulk_g2s(sx, vx + t.a0, bytes, &bar);
-            fpt_bulk_g2s(sy, vy + t.a0, bytes, &bar);
-            fpt_bulk_g2s(sz, vz + t.a0, bytes, &bar);
+    constexpr int CPW = 32 / G;                          // cells per warp
+    extern __shared__ __align__(16) unsigned char fpw_smem[];
+    float* stage = reinterpret_cast<float*>(fpw_smem);                                   // [MOM_WARPS][3][FPW_CAP]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(fpw_smem + (size_t)MOM_WARPS * 3 * FPW_CAP * sizeof(float));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int gl = lane & (G - 1), group = lane / G;
+    const int64_t cbase = ((int64_t)blockIdx.x * MOM_WARPS + warp) * CPW;
+    if (cbase >= ncell) return;
+    // the chunk's CPW + 1 cell boundaries in lanes 0..CPW
+    const int32_t cs = cell_start[min(cbase + lane, (int64_t)ncell)];
+    const fpw_range r = fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, aligned != 0);
+    const int32_t s = __shfl_sync(0xffffffffu, cs, group), e = __shfl_sync(0xffffffffu, cs, group + 1);
+    const int64_t cell = cbase + group;
+    const bool have = cell < ncell;
+    const int32_t n = have ? e - s : 0;
+    double* rec = mom + (size_t)(have ? cell : 0) * NREC;
+    if (r.staged) {
+        float* sx = stage + (size_t)(warp * 3 + 0) * FPW_CAP;
+        float* sy = stage + (size_t)(warp * 3 + 1) * FPW_CAP;
+        float* sz = stage + (size_t)(warp * 3 + 2) * FPW_CAP;
+        const uint32_t bytes = (uint32_t)r.nb * 4u;
+        if (bytes > 0) {
+            if (lane == 0) {
+                fpt_mbar_init(&bars[warp], 1);
+                fpt_mbar_expect_tx(&bars[warp], 3u * bytes);
+                fpt_bulk_g2s(sx, vx + r.a0, bytes, &bars[warp]);
+                fpt_bulk_g2s(sy, vy + r.a0, bytes, &bars[warp]);
+                fpt_bulk_g2s(sz, vz + r.a0, bytes, &bars[warp]);
+            }
+            __syncwarp();
         }
         // the (at most 3) particles beyond the last multiple of 4 of the whole array
-        for (int32_t p = t.a0 + t.nb + (int32_t)threadIdx.x; p < t.s1; p += MOM_THREADS) {
-            sx[p - t.a0] = vx[p]; sy[p - t.a0] = vy[p]; sz[p - t.a0] = vz[p];
-        }
-        if (bytes > 0) fpt_mbar_wait(&bar, 0);
-        __syncthreads();
-        bx = sx - t.a0; by = sy - t.a0; bz = sz - t.a0;
-    }
-    const int gl = threadIdx.x & (G - 1);
-    const int group = threadIdx.x / G;
-    constexpr int NGROUPS = MOM_THREADS / G;
-    for (int32_t cb = t.c0; cb < t.c1; cb += NGROUPS) {
-        if (cb + (int32_t)((threadIdx.x & ~31) / G) >= t.c1) break;      // this whole warp has no cell left
-        const int32_t cell = cb + group;
-        const bool have = cell < t.c1;
-        int32_t s = 0, n = 0;
-        if (have) { s = cell_start[cell]; n = cell_start[cell + 1] - s; }
-        mom_cell_group<G, FULL>(bx, by, bz, s, n, have, gl, mom + (size_t)(have ? cell : 0) * NREC);
+        for (int32_t p = r.a0 + r.nb + lane; p < r.s1; p += 32) { sx[p - r.a0] = vx[p]; sy[p - r.a0] = vy[p]; sz[p - r.a0] = vz[p]; }
+        if (bytes > 0) fpt_mbar_wait(&bars[warp], 0);
+        __syncwarp();
+        mom_cell_group<G, FULL>(sx - r.a0, sy - r.a0, sz - r.a0, s, n, have, gl, rec);        // shared-memory loads
+    } else {
+        mom_cell_group<G, FULL>(vx, vy, vz, s, n, have, gl, rec);                             // global loads
     }
 }
 
@@ -157,26 +164,18 @@ template <int G>
 static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
                            const int32_t* cell_start, int32_t mode, double* mom, cudaStream_t st)
 {
-    const int ntiles = fpi_ntiles(np);
+    const int cells_per_block = MOM_WARPS * (32 / G);
+    const int blocks = fp_div_up(ctx->ncell, cells_per_block);
     const int aligned = ((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0 ? 1 : 0;
-    if (mode) moments_tile_kernel<G, true><<<ntiles, MOM_THREADS, 0, st>>>(vx, vy, vz, cell_start, ctx->tile_cell, ctx->ncell, np, aligned, mom);
-    else      moments_tile_kernel<G, false><<<ntiles, MOM_THREADS, 0, st>>>(vx, vy, vz, cell_start, ctx->tile_cell, ctx->ncell, np, aligned, mom);
-}
-
-// tiles_ready: ctx->tile_cell already holds the table of this (np, cell_start)
-int fpi_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
-                     const int32_t* cell_start, int32_t mode, double* mom, bool tiles_ready, cudaStream_t st)
-{
-    int rc;
-    if (!tiles_ready && (rc = fpi_tile_table(ctx, np, cell_start, st)) != FP_OK) return rc;
-    const double ppc = (double)np / (double)ctx->ncell;
-    // group width: about 8-16 particles per lane
-    if (ppc >= 192.0)      launch_moments<16>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    else if (ppc >= 48.0)  launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    else                   launch_moments<4>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    FP_LAUNCH_OK(ctx);
-    FP_COUNT(ctx, 1);
-    return FP_OK;
+    const size_t smem = (size_t)MOM_WARPS * 3 * FPW_CAP * sizeof(float) + MOM_WARPS * sizeof(uint64_t);
+    static bool attr_set = false;                 // one flag per instantiation (G)
+    if (!attr_set) {
+        cudaFuncSetAttribute(moments_warp_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(moments_warp_kernel<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        attr_set = true;
+    }
+    if (mode) moments_warp_kernel<G, true><<<blocks, MOM_THREADS, smem, st>>>(vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
+    else      moments_warp_kernel<G, false><<<blocks, MOM_THREADS, smem, st>>>(vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
 }
 
 extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
@@ -185,6 +184,13 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     if (!ctx) return FP_ERR_ARG;
     if (np < 0 || !cell_start || !mom || (mode != 0 && mode != 1)) return fp_fail(ctx, FP_ERR_ARG, "fp_cell_moments: bad argument");
     if (np > 0 && (!vx || !vy || !vz)) return fp_fail(ctx, FP_ERR_ARG, "fp_cell_moments: null velocity pointer");
-    if (np > ctx->p.max_particles) return fp_fail(ctx, FP_ERR_STATE, "fp_cell_moments: np > max_particles");
-    return fpi_cell_moments(ctx, np, vx, vy, vz, cell_start, mode, mom, false, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    const double ppc = (double)np / (double)ctx->ncell;
+    // group width: about 8-16 particles per lane
+    if (ppc >= 192.0)      launch_moments<16>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else if (ppc >= 48.0)  launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else                   launch_moments<4>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 1);
+    return FP_OK;
 }

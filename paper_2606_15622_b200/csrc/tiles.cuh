@@ -1,15 +1,14 @@
-// tiles.cuh -- particle tiles for the per-cell kernels (moments, update).
+// tiles.cuh -- per-warp staging of contiguous particle slices in shared memory (moments, update).
 //
-// The cell-sorted particle stream is cut into tiles of about FPT_T particles that hold whole cells: tile b owns the
-// cells whose first-particle index lies in [b*FPT_T, (b+1)*FPT_T).  One CTA processes one tile: it stages the tile's
-// SoA slices in shared memory with 1D bulk asynchronous copies (cp.async.bulk -> UBLKCP, completion on an mbarrier),
-// so HBM is read once, fully coalesced, and all later passes over the cell's particles hit shared memory.
-// ntiles = np / FPT_T + 1 (the last window also catches trailing empty cells, whose start equals np).
+// The per-cell kernels give every warp 32/G consecutive cells.  Their particles are one contiguous slice of each SoA
+// array, which the warp copies into its own shared-memory buffer with 1D bulk asynchronous copies (cp.async.bulk ->
+// UBLKCP, completion on the warp's own mbarrier): HBM is read once, fully coalesced, and all later passes over the
+// cells hit shared memory.  Bulk copies need 16-byte alignment: the slice is widened to multiples of 4 elements,
+// the (at most 3) elements past the last multiple of 4 of the whole array are copied by plain loads.
 #pragma once
 #include "common.cuh"
 
-#define FPT_T 2048                 // particles per tile window
-#define FPT_CAP 2560               // staged elements per array: FPT_T - 1 + largest cell that still fits, rounded
+#define FPW_CAP 576                // staged elements per array and warp (4 cells x 144 particles)
 
 #ifdef __CUDACC__
 
@@ -55,36 +54,27 @@ __device__ __forceinline__ void fpt_fence_proxy_async()
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
-struct fpt_tile {
-    int32_t c0, c1;        // cells [c0, c1)
-    int32_t s0, s1;        // particles [s0, s1)
+struct fpw_range {
+    int32_t s0, s1;        // particles [s0, s1) of the warp's cells
     int32_t a0;            // s0 rounded down to a multiple of 4: staged element k holds particle a0 + k
     int32_t nb;            // elements covered by the bulk copies (multiple of 4), starting at a0
-    bool staged;           // false: the tile does not fit (huge cell) or the arrays are not 16-byte aligned
+    bool staged;           // false: the slice does not fit FPW_CAP or the arrays are not 16-byte aligned
 };
 
-__device__ __forceinline__ fpt_tile fpt_tile_of_block(const int32_t* __restrict__ tile_cell,
-                                                      const int32_t* __restrict__ cell_start, int32_t ncell,
-                                                      int64_t np, bool aligned)
+__device__ __forceinline__ fpw_range fpw_range_of(int32_t s0, int32_t s1, int64_t np, bool aligned)
 {
-    fpt_tile t;
-    t.c0 = tile_cell[blockIdx.x];
-    t.c1 = min(tile_cell[blockIdx.x + 1], ncell);
-    t.s0 = t.s1 = t.a0 = t.nb = 0;
-    t.staged = false;
-    if (t.c0 >= t.c1) return t;
-    t.s0 = cell_start[t.c0];
-    t.s1 = cell_start[t.c1];
-    t.a0 = t.s0 & ~3;
+    fpw_range r;
+    r.s0 = s0; r.s1 = s1;
+    r.a0 = s0 & ~3;
     const int32_t np4 = (int32_t)(np & ~(int64_t)3);
-    const int32_t end4 = min((t.s1 + 3) & ~3, np4);
-    t.nb = max(end4 - t.a0, 0);
-    t.staged = aligned && (t.s1 - t.a0) <= FPT_CAP && t.s1 > t.s0;
-    return t;
+    const int32_t end4 = min((s1 + 3) & ~3, np4);
+    r.nb = max(end4 - r.a0, 0);
+    r.staged = aligned && s1 > s0 && (s1 - r.a0) <= FPW_CAP;
+    return r;
 }
 
 #endif  // __CUDACC__
 
-// host side (tiles.cu)
-int fpi_tile_table(fp_ctx* ctx, int64_t np, const int32_t* cell_start, cudaStream_t st);
-static inline int fpi_ntiles(int64_t np) { return (int)(np / FPT_T) + 1; }
+int fpi_velocity_update(fp_ctx* ctx, int64_t np, float* vx, float* vy, float* vz, const uint32_t* pid,
+                        const int32_t* cell_start, const double* mom, int32_t mom_stride, const float* coef,
+                        const float* tau_cell, uint64_t step, uint32_t* flags, cudaStream_t st);
