@@ -133,6 +133,12 @@ __device__ __forceinline__ float fpd_uniform(uint32_t w)
     return __uint_as_float(0x3f800000u | (w >> 9)) - 0.99999994039536f;   // 1 - 2^-24
 }
 
+// packed fp32x2 arithmetic (FFMA2 / FADD2 / FMUL2 on sm_100: two fp32 operations per issue slot)
+__device__ __forceinline__ float2 fpd_fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 fpd_mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 fpd_add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 fpd_dup(float a) { return make_float2(a, a); }
+
 // 64-bit shuffle helpers
 __device__ __forceinline__ double fpd_shfl_xor(double v, int mask)
 {

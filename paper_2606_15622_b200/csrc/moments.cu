@@ -21,10 +21,14 @@
 #define MOM_CHUNK_PER_LANE 64
 
 // One cell per group of G lanes.  bx/by/bz may point to shared or global memory; particle p is at b?[p].
-template <int G, bool FULL>
+// INPLACE: the arrays are the warp's private staging copy, pass 1 overwrites v by v - v_pivot.
+template <int G, bool FULL, bool INPLACE>
 __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,
                                                bool have, int gl, double* __restrict__ rec)
 {
+    float* wx = const_cast<float*>(bx);
+    float* wy = const_cast<float*>(by);
+    float* wz = const_cast<float*>(bz);
     constexpr int NP = FULL ? 32 : 16;          // padded record length
     constexpr int NREC = FULL ? 29 : 13;
     constexpr int PER = NP / G;                 // record slots per lane after the transposing reduction
@@ -32,15 +36,30 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     // ---- pass 1: mean about the pivot
     float px = 0.f, py = 0.f, pz = 0.f;
     if (n > 0) { px = bx[s]; py = by[s]; pz = bz[s]; }
+    const float2 npx = fpd_dup(-px), npy = fpd_dup(-py), npz = fpd_dup(-pz);
     const int32_t nmax = __reduce_max_sync(0xffffffffu, n);
     double S0 = 0.0, S1 = 0.0, S2 = 0.0;
     for (int32_t c0 = 0; c0 < nmax; c0 += G * MOM_CHUNK_PER_LANE) {
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+        float2 A0 = fpd_dup(0.f), A1 = fpd_dup(0.f), A2 = fpd_dup(0.f);      // two particles per lane and step
         const int32_t cend = min(n, c0 + G * MOM_CHUNK_PER_LANE);
-#pragma unroll 4
-        for (int32_t j = c0 + gl; j < cend; j += G) {
-            a0 += bx[s + j] - px; a1 += by[s + j] - py; a2 += bz[s + j] - pz;
+        int32_t j = c0 + gl;
+#pragma unroll 2
+        for (; j + G < cend; j += 2 * G) {
+            const float2 w0 = fpd_add2(make_float2(bx[s + j], bx[s + j + G]), npx);
+            const float2 w1 = fpd_add2(make_float2(by[s + j], by[s + j + G]), npy);
+            const float2 w2 = fpd_add2(make_float2(bz[s + j], bz[s + j + G]), npz);
+            A0 = fpd_add2(A0, w0); A1 = fpd_add2(A1, w1); A2 = fpd_add2(A2, w2);
+            if (INPLACE) {      // park w = v - v_pivot for pass 2 (store pipe is idle, the FMA pipe is the bottleneck)
+                wx[s + j] = w0.x; wx[s + j + G] = w0.y; wy[s + j] = w1.x; wy[s + j + G] = w1.y;
+                wz[s + j] = w2.x; wz[s + j + G] = w2.y;
+            }
         }
+        if (j < cend) {
+            const float w0 = bx[s + j] - px, w1 = by[s + j] - py, w2 = bz[s + j] - pz;
+            A0.x += w0; A1.x += w1; A2.x += w2;
+            if (INPLACE) { wx[s + j] = w0; wy[s + j] = w1; wz[s + j] = w2; }
+        }
+        const float a0 = A0.x + A0.y, a1 = A1.x + A1.y, a2 = A2.x + A2.y;
         S0 += (double)a0; S1 += (double)a1; S2 += (double)a2;
     }
 #pragma unroll
@@ -50,34 +69,64 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     const double invn = n > 0 ? 1.0 / (double)n : 0.0;
     const double m0d = S0 * invn, m1d = S1 * invn, m2d = S2 * invn;
     const float m0 = (float)m0d, m1 = (float)m1d, m2 = (float)m2d;
+    const float2 nm0 = fpd_dup(-m0), nm1 = fpd_dup(-m1), nm2 = fpd_dup(-m2);
     // ---- pass 2: central moments
     double tot[PER];
 #pragma unroll
     for (int i = 0; i < PER; ++i) tot[i] = 0.0;
     for (int32_t c0 = 0; c0 < nmax; c0 += G * MOM_CHUNK_PER_LANE) {
-        float P0 = 0.f, P1 = 0.f, P2 = 0.f, P3 = 0.f, P4 = 0.f, P5 = 0.f;
-        float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f, t4 = 0.f, t5 = 0.f, t6 = 0.f, t7 = 0.f, t8 = 0.f, t9 = 0.f;
-        float F0 = 0.f, F1 = 0.f, F2 = 0.f, F3 = 0.f, F4 = 0.f, F5 = 0.f;
-        float g0 = 0.f, g1 = 0.f, g2 = 0.f;
+        // packed accumulators: .x and .y hold the partial sums of the two particles a lane handles per step
+        float2 P[6], T[10], F[6], Gm[3];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { P[k] = fpd_dup(0.f); F[k] = fpd_dup(0.f); }
+#pragma unroll
+        for (int k = 0; k < 10; ++k) T[k] = fpd_dup(0.f);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) Gm[k] = fpd_dup(0.f);
         const int32_t cend = min(n, c0 + G * MOM_CHUNK_PER_LANE);
-#pragma unroll 4
-        for (int32_t j = c0 + gl; j < cend; j += G) {
-            const float cx = (bx[s + j] - px) - m0, cy = (by[s + j] - py) - m1, cz = (bz[s + j] - pz) - m2;
-            const float xx = cx * cx, xy = cx * cy, xz = cx * cz, yy = cy * cy, yz = cy * cz, zz = cz * cz;
-            const float c2 = xx + yy + zz;
-            P0 += xx; P1 += xy; P2 += xz; P3 += yy; P4 += yz; P5 += zz;
-            if (FULL) {
-                t0 = fmaf(xx, cx, t0); t1 = fmaf(xx, cy, t1); t2 = fmaf(xx, cz, t2); t3 = fmaf(xy, cy, t3);
-                t4 = fmaf(xy, cz, t4); t5 = fmaf(xz, cz, t5); t6 = fmaf(yy, cy, t6); t7 = fmaf(yy, cz, t7);
-                t8 = fmaf(yz, cz, t8); t9 = fmaf(zz, cz, t9);
-                F0 = fmaf(c2, xx, F0); F1 = fmaf(c2, xy, F1); F2 = fmaf(c2, xz, F2);
-                F3 = fmaf(c2, yy, F3); F4 = fmaf(c2, yz, F4); F5 = fmaf(c2, zz, F5);
-                const float c4 = c2 * c2;
-                g0 = fmaf(c4, cx, g0); g1 = fmaf(c4, cy, g1); g2 = fmaf(c4, cz, g2);
+        int32_t j = c0 + gl;
+        const int32_t jlast = j + ((cend - j + G - 1) / G) * G;          // first index this lane does not own
+#pragma unroll 1
+        for (; j < jlast; j += 2 * G) {
+            const bool two = j + G < cend;
+            const int32_t jb = two ? j + G : j;                            // lone last particle: second half masked
+            float2 cx, cy, cz;
+            if (INPLACE) {
+                cx = fpd_add2(make_float2(bx[s + j], bx[s + jb]), nm0);
+                cy = fpd_add2(make_float2(by[s + j], by[s + jb]), nm1);
+                cz = fpd_add2(make_float2(bz[s + j], bz[s + jb]), nm2);
             } else {
-                g0 = fmaf(c2, cx, g0); g1 = fmaf(c2, cy, g1); g2 = fmaf(c2, cz, g2);      // h_i = <c^2 c_i>
+                cx = fpd_add2(fpd_add2(make_float2(bx[s + j], bx[s + jb]), npx), nm0);
+                cy = fpd_add2(fpd_add2(make_float2(by[s + j], by[s + jb]), npy), nm1);
+                cz = fpd_add2(fpd_add2(make_float2(bz[s + j], bz[s + jb]), npz), nm2);
+            }
+            if (!two) { cx.y = 0.f; cy.y = 0.f; cz.y = 0.f; }
+            const float2 xx = fpd_mul2(cx, cx), xy = fpd_mul2(cx, cy), xz = fpd_mul2(cx, cz);
+            const float2 yy = fpd_mul2(cy, cy), yz = fpd_mul2(cy, cz), zz = fpd_mul2(cz, cz);
+            const float2 c2 = fpd_add2(fpd_add2(xx, yy), zz);
+            P[0] = fpd_add2(P[0], xx); P[1] = fpd_add2(P[1], xy); P[2] = fpd_add2(P[2], xz);
+            P[3] = fpd_add2(P[3], yy); P[4] = fpd_add2(P[4], yz); P[5] = fpd_add2(P[5], zz);
+            if (FULL) {
+                T[0] = fpd_fma2(xx, cx, T[0]); T[1] = fpd_fma2(xx, cy, T[1]); T[2] = fpd_fma2(xx, cz, T[2]);
+                T[3] = fpd_fma2(xy, cy, T[3]); T[4] = fpd_fma2(xy, cz, T[4]); T[5] = fpd_fma2(xz, cz, T[5]);
+                T[6] = fpd_fma2(yy, cy, T[6]); T[7] = fpd_fma2(yy, cz, T[7]); T[8] = fpd_fma2(yz, cz, T[8]);
+                T[9] = fpd_fma2(zz, cz, T[9]);
+                F[0] = fpd_fma2(c2, xx, F[0]); F[1] = fpd_fma2(c2, xy, F[1]); F[2] = fpd_fma2(c2, xz, F[2]);
+                F[3] = fpd_fma2(c2, yy, F[3]); F[4] = fpd_fma2(c2, yz, F[4]); F[5] = fpd_fma2(c2, zz, F[5]);
+                const float2 c4 = fpd_mul2(c2, c2);
+                Gm[0] = fpd_fma2(c4, cx, Gm[0]); Gm[1] = fpd_fma2(c4, cy, Gm[1]); Gm[2] = fpd_fma2(c4, cz, Gm[2]);
+            } else {
+                Gm[0] = fpd_fma2(c2, cx, Gm[0]); Gm[1] = fpd_fma2(c2, cy, Gm[1]); Gm[2] = fpd_fma2(c2, cz, Gm[2]);   // h_i
             }
         }
+        const float P0 = P[0].x + P[0].y, P1 = P[1].x + P[1].y, P2 = P[2].x + P[2].y, P3 = P[3].x + P[3].y,
+                    P4 = P[4].x + P[4].y, P5 = P[5].x + P[5].y;
+        const float t0 = T[0].x + T[0].y, t1 = T[1].x + T[1].y, t2 = T[2].x + T[2].y, t3 = T[3].x + T[3].y,
+                    t4 = T[4].x + T[4].y, t5 = T[5].x + T[5].y, t6 = T[6].x + T[6].y, t7 = T[7].x + T[7].y,
+                    t8 = T[8].x + T[8].y, t9 = T[9].x + T[9].y;
+        const float F0 = F[0].x + F[0].y, F1 = F[1].x + F[1].y, F2 = F[2].x + F[2].y, F3 = F[3].x + F[3].y,
+                    F4 = F[4].x + F[4].y, F5 = F[5].x + F[5].y;
+        const float g0 = Gm[0].x + Gm[0].y, g1 = Gm[1].x + Gm[1].y, g2 = Gm[2].x + Gm[2].y;
         float r[NP];
         r[0] = r[1] = r[2] = r[3] = 0.f;
         r[4] = P0; r[5] = P1; r[6] = P2; r[7] = P3; r[8] = P4; r[9] = P5;
@@ -111,7 +160,9 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     }
 }
 
-// One warp = one chunk of 32/G consecutive cells, staged and processed independently of the other warps of the CTA.
+// Persistent warps: a warp owns chunks wg, wg + nwarps, ... of 32/G consecutive cells; while it reduces one chunk the
+// bulk copies of its next chunk are already in flight into the warp's other staging buffer (2-stage pipeline per
+// warp, mbarrier per stage), and the cell boundaries of the chunk after that are being fetched.
 template <int G, bool FULL>
 __global__ void __launch_bounds__(MOM_THREADS)
 moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
@@ -119,44 +170,74 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
                     double* __restrict__ mom)
 {
     constexpr int NREC = FULL ? 29 : 13;
-    constexpr int CPW = 32 / G;                          // cells per warp
+    constexpr int CPW = 32 / G;                          // cells per warp and chunk
     extern __shared__ __align__(16) unsigned char fpw_smem[];
-    float* stage = reinterpret_cast<float*>(fpw_smem);                                   // [MOM_WARPS][3][FPW_CAP]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(fpw_smem + (size_t)MOM_WARPS * 3 * FPW_CAP * sizeof(float));
+    float* stage = reinterpret_cast<float*>(fpw_smem);                                   // [MOM_WARPS][2][3][FPW_CAP]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(fpw_smem + (size_t)MOM_WARPS * 6 * FPW_CAP * sizeof(float));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gl = lane & (G - 1), group = lane / G;
-    const int64_t cbase = ((int64_t)blockIdx.x * MOM_WARPS + warp) * CPW;
-    if (cbase >= ncell) return;
-    // the chunk's CPW + 1 cell boundaries in lanes 0..CPW
-    const int32_t cs = cell_start[min(cbase + lane, (int64_t)ncell)];
-    const fpw_range r = fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, aligned != 0);
-    const int32_t s = __shfl_sync(0xffffffffu, cs, group), e = __shfl_sync(0xffffffffu, cs, group + 1);
-    const int64_t cell = cbase + group;
-    const bool have = cell < ncell;
-    const int32_t n = have ? e - s : 0;
-    double* rec = mom + (size_t)(have ? cell : 0) * NREC;
-    if (r.staged) {
-        float* sx = stage + (size_t)(warp * 3 + 0) * FPW_CAP;
-        float* sy = stage + (size_t)(warp * 3 + 1) * FPW_CAP;
-        float* sz = stage + (size_t)(warp * 3 + 2) * FPW_CAP;
+    const int64_t nchunks = ((int64_t)ncell + CPW - 1) / CPW;
+    const int64_t nw = (int64_t)gridDim.x * MOM_WARPS;
+    int64_t chunk = (int64_t)blockIdx.x * MOM_WARPS + warp;
+    if (chunk >= nchunks) return;
+    float* wbuf = stage + (size_t)warp * 6 * FPW_CAP;
+    uint64_t* wbar = bars + warp * 2;
+    if (lane == 0) { fpt_mbar_init(&wbar[0], 1); fpt_mbar_init(&wbar[1], 1); }
+    __syncwarp();
+    auto load_cs = [&](int64_t c) { return cell_start[min(c * CPW + lane, (int64_t)ncell)]; };
+    auto range_of = [&](int32_t cs) {
+        return fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, aligned != 0);
+    };
+    auto issue = [&](const fpw_range& r, int b) {
         const uint32_t bytes = (uint32_t)r.nb * 4u;
-        if (bytes > 0) {
-            if (lane == 0) {
-                fpt_mbar_init(&bars[warp], 1);
-                fpt_mbar_expect_tx(&bars[warp], 3u * bytes);
-                fpt_bulk_g2s(sx, vx + r.a0, bytes, &bars[warp]);
-                fpt_bulk_g2s(sy, vy + r.a0, bytes, &bars[warp]);
-                fpt_bulk_g2s(sz, vz + r.a0, bytes, &bars[warp]);
-            }
-            __syncwarp();
+        if (r.staged && bytes > 0 && lane == 0) {
+            float* d = wbuf + (size_t)b * 3 * FPW_CAP;
+            fpt_mbar_expect_tx(&wbar[b], 3u * bytes);
+            fpt_bulk_g2s(d, vx + r.a0, bytes, &wbar[b]);
+            fpt_bulk_g2s(d + FPW_CAP, vy + r.a0, bytes, &wbar[b]);
+            fpt_bulk_g2s(d + 2 * FPW_CAP, vz + r.a0, bytes, &wbar[b]);
         }
-        // the (at most 3) particles beyond the last multiple of 4 of the whole array
-        for (int32_t p = r.a0 + r.nb + lane; p < r.s1; p += 32) { sx[p - r.a0] = vx[p]; sy[p - r.a0] = vy[p]; sz[p - r.a0] = vz[p]; }
-        if (bytes > 0) fpt_mbar_wait(&bars[warp], 0);
-        __syncwarp();
-        mom_cell_group<G, FULL>(sx - r.a0, sy - r.a0, sz - r.a0, s, n, have, gl, rec);        // shared-memory loads
-    } else {
-        mom_cell_group<G, FULL>(vx, vy, vz, s, n, have, gl, rec);                             // global loads
+    };
+    int32_t cs_cur = load_cs(chunk);
+    int64_t nxt = chunk + nw;
+    int32_t cs_nxt = nxt < nchunks ? load_cs(nxt) : 0;
+    fpw_range r_cur = range_of(cs_cur);
+    issue(r_cur, 0);
+    int b = 0;
+    uint32_t phase = 0;
+    while (true) {
+        fpw_range r_nxt = r_cur;
+        if (nxt < nchunks) {
+            r_nxt = range_of(cs_nxt);
+            __syncwarp();                                   // every lane is done reading buffer b^1 (previous chunk)
+            issue(r_nxt, b ^ 1);
+        }
+        const int64_t nxt2 = nxt + nw;
+        const int32_t cs_nxt2 = nxt2 < nchunks ? load_cs(nxt2) : 0;
+        // ---- the current chunk
+        const int32_t s = __shfl_sync(0xffffffffu, cs_cur, group), e = __shfl_sync(0xffffffffu, cs_cur, group + 1);
+        const int64_t cell = chunk * CPW + group;
+        const bool have = cell < ncell;
+        const int32_t n = have ? e - s : 0;
+        double* rec = mom + (size_t)(have ? cell : 0) * NREC;
+        if (r_cur.staged) {
+            float* sx = wbuf + (size_t)b * 3 * FPW_CAP;
+            float* sy = sx + FPW_CAP;
+            float* sz = sy + FPW_CAP;
+            // the (at most 3) particles beyond the last multiple of 4 of the whole array
+            for (int32_t p = r_cur.a0 + r_cur.nb + lane; p < r_cur.s1; p += 32) {
+                sx[p - r_cur.a0] = vx[p]; sy[p - r_cur.a0] = vy[p]; sz[p - r_cur.a0] = vz[p];
+            }
+            if (r_cur.nb > 0) { fpt_mbar_wait(&wbar[b], (phase >> b) & 1u); phase ^= 1u << b; }
+            __syncwarp();
+            mom_cell_group<G, FULL, true>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, s, n, have, gl, rec);   // shared-memory loads
+        } else {
+            mom_cell_group<G, FULL, false>(vx, vy, vz, s, n, have, gl, rec);                                    // global loads
+        }
+        if (nxt >= nchunks) break;
+        chunk = nxt; cs_cur = cs_nxt; r_cur = r_nxt;
+        nxt = nxt2; cs_nxt = cs_nxt2;
+        b ^= 1;
     }
 }
 
@@ -165,15 +246,18 @@ static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float
                            const int32_t* cell_start, int32_t mode, double* mom, cudaStream_t st)
 {
     const int cells_per_block = MOM_WARPS * (32 / G);
-    const int blocks = fp_div_up(ctx->ncell, cells_per_block);
     const int aligned = ((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0 ? 1 : 0;
-    const size_t smem = (size_t)MOM_WARPS * 3 * FPW_CAP * sizeof(float) + MOM_WARPS * sizeof(uint64_t);
-    static bool attr_set = false;                 // one flag per instantiation (G)
-    if (!attr_set) {
+    const size_t smem = (size_t)MOM_WARPS * 6 * FPW_CAP * sizeof(float) + MOM_WARPS * 2 * sizeof(uint64_t);
+    static int occ = 0;                           // resident CTAs per SM, one value per instantiation (G)
+    if (occ == 0) {
         cudaFuncSetAttribute(moments_warp_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         cudaFuncSetAttribute(moments_warp_kernel<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_set = true;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, moments_warp_kernel<G, true>, MOM_THREADS, smem);
+        if (occ < 1) occ = 1;
     }
+    const int want = fp_div_up(ctx->ncell, cells_per_block);
+    const int cap = ctx->num_sms * occ;
+    const int blocks = want < cap ? want : cap;
     if (mode) moments_warp_kernel<G, true><<<blocks, MOM_THREADS, smem, st>>>(vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
     else      moments_warp_kernel<G, false><<<blocks, MOM_THREADS, smem, st>>>(vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
 }

@@ -8,7 +8,7 @@
 #pragma once
 #include "common.cuh"
 
-#define FPW_CAP 576                // staged elements per array and warp (4 cells x 144 particles)
+#define FPW_CAP 512                // staged elements per array, warp and stage (4 cells x 128 particles)
 
 #ifdef __CUDACC__
 
