@@ -54,7 +54,7 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && sms > 0) c->num_sms = sms;
     const size_t n = (size_t)(q.max_particles > 0 ? q.max_particles : 1);
-    const size_t nblocks = (n + 2047) / 2048;
+    const size_t nblocks = (n + SORT_TILE - 1) / SORT_TILE;
     c->block_hist_elems = 512 * nblocks;
     bool ok = cudaMalloc((void**)&c->key_a, n * 4) == cudaSuccess && cudaMalloc((void**)&c->key_b, n * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->idx_a, n * 4) == cudaSuccess && cudaMalloc((void**)&c->idx_b, n * 4) == cudaSuccess &&
@@ -119,7 +119,7 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
     if ((rc = fpi_stream_walls(ctx, np, x_a, y_a, vx_a, vy_a, vz_a, pid_a, step, ctx->key_b, st)) != FP_OK) return rc;
     fp_mark(ctx, 1, st);
     // a2 (records mark 2 between the key sort and the payload gather)
-    if ((rc = fpi_sort_with_keys(ctx, np, ctx->key_b, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b,
+    if ((rc = fpi_sort_with_keys(ctx, np, ctx->key_b, false, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b,
                                  cell_start, nullptr, st)) != FP_OK) return rc;
     fp_mark(ctx, 3, st);
     const float* tau_use = nullptr;

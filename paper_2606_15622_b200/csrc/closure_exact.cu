@@ -12,7 +12,7 @@
 // memory (stride 29 doubles is bank-conflict free), each thread scales its record in registers, writes its augmented
 // 9x10 system to shared memory as [entry][thread] (conflict free, dynamic row index = free pivoting without register
 // selects) and eliminates in place.  The system never touches HBM: 232 B/cell in, 40 B/cell out.
-#include "common.cuh"
+#include "tiles.cuh"
 
 #define CE_TPB 64
 
@@ -78,8 +78,8 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
     const int tid = threadIdx.x;
     const int64_t cell0 = (int64_t)blockIdx.x * CE_TPB;
     const int ncb = (int)min((int64_t)CE_TPB, (int64_t)ncell - cell0);
-    for (int e = tid; e < ncb * 29; e += CE_TPB) recs[e] = mom[(size_t)cell0 * 29 + e];
-    __syncthreads();
+    __shared__ __align__(8) uint64_t bar;
+    fpt_block_stage(recs, mom + (size_t)cell0 * 29, (uint32_t)ncb * 29u * 8u, &bar);
     if (tid >= ncb) return;
     const int64_t cell = cell0 + tid;
     const double* rec = recs + tid * 29;

@@ -9,6 +9,12 @@
 #include "../../include/fpcl.h"
 
 #define FPCL_MAX_LAYERS 8
+// radix sort tiling (sort.cu; the key kernel also produces the first digit histogram per tile)
+#define SORT_THREADS 256
+#define SORT_WARPS (SORT_THREADS / 32)
+#define SORT_ITEMS 16                                    // items per thread
+#define SORT_TILE (SORT_THREADS * SORT_ITEMS)            // 4096 items per block
+#define SORT_MAX_BINS 512
 #define FPCL_NUM_SMS_DEFAULT 148
 
 // ---------------------------------------------------------------------------------------------------------
@@ -88,7 +94,8 @@ static inline int fp_fail(fp_ctx* ctx, int code, const char* msg)
 static inline int fp_div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // internal entry points shared between translation units (not exported)
-int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
+int fpi_sort_digit_bits(const fp_ctx* ctx);           // width of one radix digit for this grid
+int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0_ready,
                        const float* x, const float* y, const float* vx, const float* vy, const float* vz,
                        const uint32_t* pid, float* x_out, float* y_out, float* vx_out, float* vy_out,
                        float* vz_out, uint32_t* pid_out, int32_t* cell_start, uint32_t* perm, cudaStream_t st);

@@ -7,22 +7,32 @@
 // The payload (x, y, vx, vy, vz, pid) is gathered once at the end through the final permutation.
 #include "common.cuh"
 
-#define SORT_THREADS 256
-#define SORT_WARPS (SORT_THREADS / 32)
-#define SORT_ITEMS 8                                     // items per thread
-#define SORT_TILE (SORT_THREADS * SORT_ITEMS)            // 2048 items per block
-#define SORT_MAX_BINS 512
-
-__global__ void __launch_bounds__(256)
+// cell keys of tile blockIdx.x plus the tile's histogram of the first radix digit
+__global__ void __launch_bounds__(SORT_THREADS)
 key_kernel(int64_t np, const float* __restrict__ x, const float* __restrict__ y, uint32_t* __restrict__ keys,
-           int32_t nx, int32_t ny, float x0, float y0, float inv_dx, float inv_dy)
+           int32_t nx, int32_t ny, float x0, float y0, float inv_dx, float inv_dy,
+           uint32_t* __restrict__ block_hist, int nblocks, int bins)
 {
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += stride) {
-        const int32_t ix = fpd_axis_index(x[p], x0, inv_dx, nx);
-        const int32_t iy = (ny > 1) ? fpd_axis_index(y[p], y0, inv_dy, ny) : 0;
-        keys[p] = (uint32_t)(iy * nx + ix);
+    __shared__ uint32_t h[SORT_MAX_BINS];
+    for (int b = threadIdx.x; b < bins; b += SORT_THREADS) h[b] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+    const uint32_t mask = (uint32_t)bins - 1u;
+#pragma unroll 4
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        const int64_t p = base + i * SORT_THREADS + threadIdx.x;
+        const bool valid = p < np;
+        uint32_t key = 0;
+        if (valid) {
+            const int32_t ix = fpd_axis_index(x[p], x0, inv_dx, nx);
+            const int32_t iy = (ny > 1) ? fpd_axis_index(y[p], y0, inv_dy, ny) : 0;
+            key = (uint32_t)(iy * nx + ix);
+            keys[p] = key;
+        }
+        if (valid) atomicAdd(&h[key & mask], 1u);
     }
+    __syncthreads();
+    for (int b = threadIdx.x; b < bins; b += SORT_THREADS) block_hist[(size_t)b * nblocks + blockIdx.x] = h[b];
 }
 
 // per-tile digit histogram: block_hist[bin * nblocks + block]
@@ -44,24 +54,28 @@ hist_kernel(int64_t np, const uint32_t* __restrict__ keys, uint32_t* __restrict_
     for (int b = threadIdx.x; b < bins; b += SORT_THREADS) block_hist[(size_t)b * nblocks + blockIdx.x] = h[b];
 }
 
-// one warp per digit value: exclusive scan of that digit's counts over tiles (in place) and the digit total
-__global__ void __launch_bounds__(128)
-scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_total, int nblocks, int bins)
+// one block per digit value: exclusive scan of that digit's counts over tiles (in place) and the digit total
+__global__ void __launch_bounds__(256)
+scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_total, int nblocks)
 {
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (warp >= bins) return;
-    uint32_t* row = block_hist + (size_t)warp * nblocks;
-    uint32_t carry = 0;
-    for (int b0 = 0; b0 < nblocks; b0 += 32) {
-        const int b = b0 + lane;
-        const uint32_t v = (b < nblocks) ? row[b] : 0u;
-        uint32_t s = v;
+    __shared__ uint32_t wsum[8];
+    uint32_t* row = block_hist + (size_t)blockIdx.x * nblocks;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int per = (nblocks + 255) / 256;
+    const int beg = min(tid * per, nblocks), end = min(beg + per, nblocks);
+    uint32_t sum = 0;
+    for (int i = beg; i < end; ++i) sum += row[i];
+    uint32_t incl = sum;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, s, d); if (lane >= d) s += t; }
-        if (b < nblocks) row[b] = carry + s - v;
-        carry += __shfl_sync(0xffffffffu, s, 31);
-    }
-    if (lane == 0) bin_total[warp] = carry;
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t wbase = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { if (w < warp) wbase += wsum[w]; total += wsum[w]; }
+    uint32_t run = wbase + incl - sum;
+    for (int i = beg; i < end; ++i) { const uint32_t v = row[i]; row[i] = run; run += v; }
+    if (tid == 0) bin_total[blockIdx.x] = total;
 }
 
 // stable scatter of one tile.  Warp w owns items [w*256, (w+1)*256) of the tile in warp-striped order
@@ -139,20 +153,11 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
     }
 }
 
-// cell_start from the sorted keys: cell_start[k] = first position whose key >= k; cell_start[ncell] = np.
+// payload permute fused with cell_start from the sorted keys: cell_start[k] = first position whose key >= k,
+// cell_start[ncell] = np.  Thread k owns the boundary between positions k-1 and k (and the last one also np).
 __global__ void __launch_bounds__(256)
-cell_start_kernel(int64_t np, const uint32_t* __restrict__ skeys, int32_t ncell, int32_t* __restrict__ cell_start)
-{
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p <= np; p += stride) {
-        const int64_t lo = (p == 0) ? 0 : (int64_t)skeys[p - 1] + 1;
-        const int64_t hi = (p == np) ? (int64_t)ncell : (int64_t)skeys[p];
-        for (int64_t k = lo; k <= hi; ++k) cell_start[k] = (int32_t)p;
-    }
-}
-
-__global__ void __launch_bounds__(256)
-gather_kernel(int64_t np, const uint32_t* __restrict__ perm,
+gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ skeys, int32_t ncell,
+              int32_t* __restrict__ cell_start,
               const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ vx,
               const float* __restrict__ vy, const float* __restrict__ vz, const uint32_t* __restrict__ pid,
               float* __restrict__ xo, float* __restrict__ yo, float* __restrict__ vxo, float* __restrict__ vyo,
@@ -161,7 +166,11 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm,
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < np; k += stride) {
         const uint32_t s = perm[k];
+        const uint32_t key = skeys[k];
+        const int64_t lo = (k == 0) ? 0 : (int64_t)skeys[k - 1] + 1;
         xo[k] = x[s]; yo[k] = y[s]; vxo[k] = vx[s]; vyo[k] = vy[s]; vzo[k] = vz[s]; pido[k] = pid[s];
+        for (int64_t c = lo; c <= (int64_t)key; ++c) cell_start[c] = (int32_t)k;
+        if (k == np - 1) for (int64_t c = (int64_t)key + 1; c <= (int64_t)ncell; ++c) cell_start[c] = (int32_t)np;
     }
 }
 
@@ -171,7 +180,14 @@ __global__ void zero_i32_kernel(int32_t* a, int64_t n)
     if (i < n) a[i] = 0;
 }
 
-int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
+int fpi_sort_digit_bits(const fp_ctx* ctx)
+{
+    const int bits = ctx->key_bits < 1 ? 1 : ctx->key_bits;
+    const int passes = (bits + 8) / 9;
+    return (bits + passes - 1) / passes;                 // <= 9
+}
+
+int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0_ready,
                        const float* x, const float* y, const float* vx, const float* vy, const float* vz,
                        const uint32_t* pid, float* x_out, float* y_out, float* vx_out, float* vy_out,
                        float* vz_out, uint32_t* pid_out, int32_t* cell_start, uint32_t* perm, cudaStream_t st)
@@ -187,7 +203,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
     const int nblocks = fp_div_up(np, SORT_TILE);
     const int bits = ctx->key_bits < 1 ? 1 : ctx->key_bits;
     const int passes = (bits + 8) / 9;
-    const int dbits = (bits + passes - 1) / passes;          // <= 9
+    const int dbits = fpi_sort_digit_bits(ctx);
     const int bins = 1 << dbits;
     if ((size_t)bins * nblocks > ctx->block_hist_elems) return fp_fail(ctx, FP_ERR_STATE, "sort scratch too small");
     const uint32_t* kin = keys;
@@ -196,26 +212,28 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys,
     uint32_t* iout = ctx->idx_a;
     for (int pass = 0; pass < passes; ++pass) {
         const int shift = pass * dbits;
-        hist_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, kin, ctx->block_hist, nblocks, shift, bins);
-        scan_rows_kernel<<<fp_div_up((int64_t)bins * 32, 128), 128, 0, st>>>(ctx->block_hist, ctx->bin_total, nblocks, bins);
+        if (!(pass == 0 && hist0_ready)) {
+            hist_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, kin, ctx->block_hist, nblocks, shift, bins);
+            FP_COUNT(ctx, 1);
+        }
+        scan_rows_kernel<<<bins, 256, 0, st>>>(ctx->block_hist, ctx->bin_total, nblocks);
         if (pass == 0)
             scatter_kernel<true><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, ctx->block_hist, ctx->bin_total, nblocks, shift, bins);
         else
             scatter_kernel<false><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, ctx->block_hist, ctx->bin_total, nblocks, shift, bins);
         FP_LAUNCH_OK(ctx);
-        FP_COUNT(ctx, 3);
+        FP_COUNT(ctx, 2);
         kin = kout; iin = iout;
         kout = (kout == ctx->key_a) ? ctx->key_b : ctx->key_a;
         iout = (iout == ctx->idx_a) ? ctx->idx_b : ctx->idx_a;
     }
-    const int64_t cap = (int64_t)ctx->num_sms * 16;
-    int64_t want = (np + 1 + 255) / 256;
-    cell_start_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, kin, ncell, cell_start);
     fp_mark(ctx, 2, st);
-    want = (np + 255) / 256;
-    gather_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, iin, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out, pid_out);
+    const int64_t cap = (int64_t)ctx->num_sms * 16;
+    const int64_t want = (np + 255) / 256;
+    gather_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
+                                                                 x_out, y_out, vx_out, vy_out, vz_out, pid_out);
     FP_LAUNCH_OK(ctx);
-    FP_COUNT(ctx, 2);
+    FP_COUNT(ctx, 1);
     if (perm) FP_CUDA_OK(ctx, cudaMemcpyAsync(perm, iin, (size_t)np * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
     return FP_OK;
 }
@@ -236,13 +254,13 @@ extern "C" int fp_sort_by_cell(fp_ctx* ctx, int64_t np,
     cudaStream_t st = (cudaStream_t)stream;
     if (np > 0) {
         const fp_params& q = ctx->p;
-        const int64_t cap = (int64_t)ctx->num_sms * 16;
-        const int64_t want = (np + 255) / 256;
-        key_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, x, y, ctx->key_b, q.nx, q.ny, q.x0, q.y0, ctx->inv_dx, ctx->inv_dy);
+        const int nblocks = fp_div_up(np, SORT_TILE);
+        key_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, x, y, ctx->key_b, q.nx, q.ny, q.x0, q.y0, ctx->inv_dx, ctx->inv_dy,
+                                                    ctx->block_hist, nblocks, 1 << fpi_sort_digit_bits(ctx));
         FP_LAUNCH_OK(ctx);
         FP_COUNT(ctx, 1);
     }
     // keys live in key_b; the first pass writes key_a, so the ping-pong never overwrites its own input
-    return fpi_sort_with_keys(ctx, np, ctx->key_b, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out,
+    return fpi_sort_with_keys(ctx, np, ctx->key_b, np > 0, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out,
                               pid_out, cell_start, perm, st);
 }

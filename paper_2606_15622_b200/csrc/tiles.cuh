@@ -54,6 +54,26 @@ __device__ __forceinline__ void fpt_fence_proxy_async()
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
+// Block-wide staging of a contiguous slab (e.g. the moment records of the block's cells): one bulk copy when the
+// slab is 16-byte aligned, plain loads for the remainder.  Ends with __syncthreads().  `bar` must be a block-shared
+// mbarrier used for nothing else.
+__device__ __forceinline__ void fpt_block_stage(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    const bool aligned = ((reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst)) & 15u) == 0;
+    const uint32_t bulk = aligned ? (bytes & ~15u) : 0u;
+    if (threadIdx.x == 0 && bulk > 0) {
+        fpt_mbar_init(bar, 1);
+        fpt_mbar_expect_tx(bar, bulk);
+        fpt_bulk_g2s(dst, src, bulk, bar);
+    }
+    for (uint32_t o = bulk + threadIdx.x * 4u; o < bytes; o += blockDim.x * 4u)
+        *reinterpret_cast<uint32_t*>(static_cast<unsigned char*>(dst) + o) =
+            *reinterpret_cast<const uint32_t*>(static_cast<const unsigned char*>(src) + o);
+    __syncthreads();                                     // barrier initialised and visible to every thread
+    if (bulk > 0) fpt_mbar_wait(bar, 0);
+    __syncthreads();
+}
+
 struct fpw_range {
     int32_t s0, s1;        // particles [s0, s1) of the warp's cells
     int32_t a0;            // s0 rounded down to a multiple of 4: staged element k holds particle a0 + k
