@@ -136,6 +136,12 @@ int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell 
 int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell /* nullable */,
                    const fp_mlp* h_mlp, float relax_w, float* coef, uint32_t* flags, void* stream);
 
+/* Surrogate kernel choice.  enable = 1 (default): networks of shape [13|16]-64-64-64-9 run on the tensor cores
+ * (mma.sync TF32 with 3xTF32 error compensation; agrees with an fp64 forward pass to ~1e-5 of the output scale --
+ * north_star allows 3e-3 for TF32); every other shape, and every shape when enable = 0, runs the plain fp32-FMA
+ * kernel (1e-5).  The environment variable FPCL_MLP_FP32=1 sets enable = 0 at fp_create. */
+int fp_set_mlp_tensor_cores(fp_ctx* ctx, int32_t enable);
+
 /* a6 -- FP velocity update, in place on cell-sorted vx, vy, vz (Eq. 13-15 :150-181; R5, R6).
  * step is the Philox counter word for time.  flags [ncell] are OR-ed with FP_FLAG_ALPHA / FP_FLAG_SKIPPED. */
 int fp_velocity_update(fp_ctx* ctx, int64_t np, float* vx, float* vy, float* vz, const uint32_t* pid,

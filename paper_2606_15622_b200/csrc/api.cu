@@ -2,6 +2,7 @@
 // :250-270): stream -> walls -> sort -> moments -> closure -> update, all on one stream with no host
 // synchronisation and no allocation inside (scratch lives in fp_ctx).
 #include <math.h>
+#include <stdlib.h>
 #include <new>
 
 #include "tiles.cuh"
@@ -18,7 +19,7 @@ static void fp_free_all(fp_ctx* c)
     cudaFree(c->block_hist); cudaFree(c->bin_total); cudaFree(c->cellc);
     for (int s = 0; s < 2; ++s) { for (int k = 0; k < 5; ++k) cudaFree(c->hs_f[s][k]); cudaFree(c->hs_pid[s]); }
     cudaFree(c->hs_mom); cudaFree(c->hs_coef); cudaFree(c->hs_flags); cudaFree(c->hs_cell_start);
-    cudaFree(c->mlp.blob);
+    cudaFree(c->mlp.blob); cudaFree(c->mlp.tc_frags);
 }
 
 static void fp_timing_free(fp_ctx* c);
@@ -37,6 +38,7 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
     if (!c) return FP_ERR_STATE;
     c->err[0] = 0;
     c->p = q;
+    { const char* e = getenv("FPCL_MLP_FP32"); c->mlp_force_fp32 = e && e[0] == '1'; }
     c->ncell = q.nx * q.ny;
     int bits = 0;
     while (((int64_t)1 << bits) < (int64_t)c->ncell) ++bits;

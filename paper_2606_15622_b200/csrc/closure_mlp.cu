@@ -31,6 +31,8 @@ struct mlp_src {
 
 static inline int pad8(int v) { return (v + 7) & ~7; }
 
+#include "mlp_tc.cuh"
+
 // repack caller weights [out][in] -> blob Wt[in][out_pad], bias[out_pad] (zero padded), scalers appended
 __global__ void mlp_pack_kernel(const __grid_constant__ mlp_desc D, const __grid_constant__ mlp_src S,
                                 float* __restrict__ blob)
@@ -163,6 +165,13 @@ mlp_kernel(const double* __restrict__ mom, int32_t stride, const float* __restri
     flags[cell] = flag;
 }
 
+extern "C" int fp_set_mlp_tensor_cores(fp_ctx* ctx, int32_t enable)
+{
+    if (!ctx) return FP_ERR_ARG;
+    ctx->mlp_force_fp32 = (enable == 0);
+    return FP_OK;
+}
+
 extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell,
                               const fp_mlp* h_mlp, float relax_w, float* coef, uint32_t* flags, void* stream)
 {
@@ -203,6 +212,31 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
     S.x_mean = M.x_mean; S.x_scale = M.x_scale; S.y_mean = M.y_mean; S.y_scale = M.y_scale;
     cudaStream_t st = (cudaStream_t)stream;
     fp_mlp_dev& C = ctx->mlp;
+    // ---- tensor-core path for the benchmark shape [13|16]-64-64-64-9
+    if (!ctx->mlp_force_fp32 && M.n_layers == 4 && D.dims[1] == TC_H && D.dims[2] == TC_H && D.dims[3] == TC_H) {
+        const size_t fbytes = (size_t)TC_FRAGS * sizeof(float4) + (size_t)TC_MISC * sizeof(float);
+        if (!C.tc_frags) FP_CUDA_OK(ctx, cudaMalloc((void**)&C.tc_frags, fbytes));
+        float4* frags = reinterpret_cast<float4*>(C.tc_frags);
+        float* misc = C.tc_frags + (size_t)TC_FRAGS * 4;
+        mlp_tc_pack_kernel<<<20, 256, 0, st>>>(S, D.dims[0], frags, misc);
+        tc_params P;
+        P.stride = mom_stride; P.feature_set = M.feature_set; P.act = M.act; P.min_count = ctx->p.min_count_mlp;
+        P.ncell = ctx->ncell; P.nin = D.dims[0]; P.tau_scalar = ctx->p.tau; P.n_scale = M.n_scale;
+        P.theta_ref = M.theta_ref; P.relax_w = relax_w;
+        const size_t smem = fbytes + (size_t)TC_WARPS * 16 * 17 * sizeof(float);
+        static int occ = 0;
+        if (occ == 0) {
+            FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mlp_tc_kernel, TC_THREADS, smem);
+            if (occ < 1) occ = 1;
+        }
+        const int want = fp_div_up(fp_div_up(ctx->ncell, 16), TC_WARPS);
+        const int cap = ctx->num_sms * occ;
+        mlp_tc_kernel<<<want < cap ? want : cap, TC_THREADS, smem, st>>>(mom, tau_cell, frags, misc, coef, flags, P);
+        FP_LAUNCH_OK(ctx);
+        FP_COUNT(ctx, 2);
+        return FP_OK;
+    }
     if (C.blob_floats < (size_t)off) {           // grow the packed-parameter scratch (stream-ordered)
         if (C.blob) FP_CUDA_OK(ctx, cudaFreeAsync(C.blob, st));
         C.blob = nullptr; C.blob_floats = 0;

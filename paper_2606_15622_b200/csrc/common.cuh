@@ -25,6 +25,7 @@ struct fp_mlp_dev {                 // uploaded copy of the caller's MLP (fp_clo
     int32_t  dims[FPCL_MAX_LAYERS + 1] = {0};
     int32_t  act = 0, feature_set = 0;
     float    n_scale = 1.f, theta_ref = 0.5f;
+    float*   tc_frags = nullptr;    // device: packed 3xTF32 mma fragments + biases/scalers (mlp_tc.cuh)
     float*   blob = nullptr;        // device: [W0 | b0 | W1 | b1 | ... | x_mean | x_scale | y_mean | y_scale]
     size_t   blob_floats = 0;
     size_t   w_off[FPCL_MAX_LAYERS] = {0}, b_off[FPCL_MAX_LAYERS] = {0};
@@ -58,6 +59,7 @@ struct fp_ctx {
     int32_t  *hs_cell_start = nullptr;
     bool      hs_ready = false;
     fp_mlp_dev mlp;
+    bool      mlp_force_fp32 = false;   // FPCL_MLP_FP32=1: always use the plain-FMA surrogate kernel
     // measurement hooks
     uint64_t  launches = 0;
     cudaEvent_t* t_ev = nullptr;     // [t_max * (FP_NSTAGES + 1)]

@@ -1,0 +1,255 @@
+// mlp_tc.cuh -- tensor-core path of the fused MLP surrogate for the benchmark shape [13|16]-64-64-64-9
+// (BASELINE.json config 1).  Included by closure_mlp.cu only.
+//
+// One warp = one tile of 16 cells = the M dimension of mma.sync.m16n8k8 (TF32 inputs, fp32 accumulate).  To keep
+// fp32-level accuracy (tolerance 1e-5, not the 3e-3 a plain TF32 product would need) every product is split
+// "3xTF32": x = x_hi + x_lo with both parts rounded to TF32, and A.B ~= A_lo.B_hi + A_hi.B_lo + A_hi.B_hi.
+// The whole network stays in registers: the accumulator fragment of one layer is, after bias and activation, the
+// A fragment of the next one.  That works without any shuffle because the K index of a layer is a summation index
+// and may be permuted: accumulator columns (2t, 2t+1) of n-tile j become K slots (t, t+4) of k-step j, and the
+// weights are pre-packed in exactly that order (and already split into hi/lo) by mlp_tc_pack_kernel, one float4
+// {b0_hi, b1_hi, b0_lo, b1_lo} per (layer, k-step, n-tile, lane): a conflict-free 128-bit shared-memory load per mma
+// triple.  Features, standardisation, fallback policy and under-relaxation are the same as in the fp32 kernel.
+#pragma once
+
+#define TC_WARPS 8
+#define TC_THREADS (TC_WARPS * 32)
+#define TC_H 64                                  // hidden width
+// float4 fragments per layer: k-steps x n-tiles x 32 lanes
+#define TC_F1 (2 * 8 * 32)                       // layer 1: K = 16 (13 or 16 inputs, zero padded), N = 64
+#define TC_F2 (8 * 8 * 32)                       // layers 2, 3: K = 64, N = 64
+#define TC_F4 (8 * 2 * 32)                       // head: K = 64, N = 16 (9 outputs, zero padded)
+#define TC_FRAGS (TC_F1 + 2 * TC_F2 + TC_F4)     // 5120 float4 = 80 KB
+#define TC_MISC (4 * TC_H + 64)                  // biases of 4 layers (padded to 64) + x_mean, x_scale, y_mean, y_scale (16 each)
+
+__device__ __forceinline__ uint32_t tc_tf32(float x)
+{
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ void tc_split(float x, uint32_t& hi, uint32_t& lo)
+{
+    hi = tc_tf32(x);
+    lo = tc_tf32(x - __uint_as_float(hi));
+}
+__device__ __forceinline__ void tc_mma(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// Pack caller weights W[l] ([out][in] row-major) into mma B fragments, split hi/lo.  Fragment (l, j, n, lane):
+// g = lane / 4, t = lane % 4, out = 8 n + g, in0 = 8 j + 2 t, in1 = in0 + 1  ->  {hi(W[out][in0]), hi(W[out][in1]),
+// lo(W[out][in0]), lo(W[out][in1])}, zero outside the layer's true shape.  misc: biases and scalers.
+__global__ void mlp_tc_pack_kernel(const __grid_constant__ mlp_src S, int32_t nin, float4* __restrict__ frags,
+                                   float* __restrict__ misc)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int e = tid; e < TC_FRAGS; e += nth) {
+        int l, r = e;
+        if (r < TC_F1) l = 0;
+        else if ((r -= TC_F1) < TC_F2) l = 1;
+        else if ((r -= TC_F2) < TC_F2) l = 2;
+        else { r -= TC_F2; l = 3; }
+        const int NT = (l == 3) ? 2 : 8;
+        const int ni = (l == 0) ? nin : TC_H, no = (l == 3) ? 9 : TC_H;
+        const int lane = r & 31, n = (r >> 5) % NT, j = (r >> 5) / NT;
+        const int g = lane >> 2, t = lane & 3;
+        const int o = 8 * n + g, i0 = 8 * j + 2 * t, i1 = i0 + 1;
+        const float w0 = (o < no && i0 < ni) ? S.W[l][(size_t)o * ni + i0] : 0.0f;
+        const float w1 = (o < no && i1 < ni) ? S.W[l][(size_t)o * ni + i1] : 0.0f;
+        uint32_t h0, l0, h1, l1;
+        tc_split(w0, h0, l0);
+        tc_split(w1, h1, l1);
+        frags[e] = make_float4(__uint_as_float(h0), __uint_as_float(h1), __uint_as_float(l0), __uint_as_float(l1));
+    }
+    for (int e = tid; e < TC_MISC; e += nth) {
+        float v = 0.0f;
+        if (e < 4 * TC_H) {
+            const int l = e / TC_H, o = e % TC_H;
+            const int no = (l == 3) ? 9 : TC_H;
+            v = (o < no) ? S.b[l][o] : 0.0f;
+        } else {
+            const int q = (e - 4 * TC_H) / 16, i = (e - 4 * TC_H) % 16;
+            if (q == 0) v = (i < nin) ? S.x_mean[i] : 0.0f;
+            else if (q == 1) v = (i < nin) ? S.x_scale[i] : 1.0f;
+            else if (q == 2) v = (i < 9) ? S.y_mean[i] : 0.0f;
+            else v = (i < 9) ? S.y_scale[i] : 0.0f;
+        }
+        misc[e] = v;
+    }
+}
+
+// One dense layer on a 16-cell tile.  ahi/alo: KS k-steps of A fragments (hi and lo parts); c: NT accumulator tiles,
+// initialised with the bias.  wf points at the layer's fragments in shared memory.
+template <int KS, int NT>
+__device__ __forceinline__ void tc_layer(const uint32_t (&ahi)[8][4], const uint32_t (&alo)[8][4], float (&c)[8][4],
+                                         const float4* __restrict__ wf, const float* __restrict__ bias, int lane)
+{
+    const int t = lane & 3;
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+        const float b0 = bias[8 * n + 2 * t], b1 = bias[8 * n + 2 * t + 1];
+        c[n][0] = b0; c[n][1] = b1; c[n][2] = b0; c[n][3] = b1;
+    }
+#pragma unroll
+    for (int j = 0; j < KS; ++j) {
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+            const float4 w = wf[(j * NT + n) * 32 + lane];
+            const uint32_t bh0 = __float_as_uint(w.x), bh1 = __float_as_uint(w.y);
+            const uint32_t bl0 = __float_as_uint(w.z), bl1 = __float_as_uint(w.w);
+            tc_mma(c[n], alo[j], bh0, bh1);          // small terms first
+            tc_mma(c[n], ahi[j], bl0, bl1);
+            tc_mma(c[n], ahi[j], bh0, bh1);
+        }
+    }
+}
+
+// activation on the accumulators and conversion into the next layer's A fragments (K slot t <- column 2t,
+// slot t+4 <- column 2t+1: a0 = c0, a1 = c2, a2 = c1, a3 = c3)
+__device__ __forceinline__ void tc_activate(const float (&c)[8][4], uint32_t (&ahi)[8][4], uint32_t (&alo)[8][4], int act)
+{
+#pragma unroll
+    for (int n = 0; n < 8; ++n) {
+        float v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const float s = c[n][q];
+            v[q] = (act == 0) ? s / (1.0f + expf(-s)) : fmaxf(s, 0.0f);
+        }
+        tc_split(v[0], ahi[n][0], alo[n][0]);
+        tc_split(v[2], ahi[n][1], alo[n][1]);
+        tc_split(v[1], ahi[n][2], alo[n][2]);
+        tc_split(v[3], ahi[n][3], alo[n][3]);
+    }
+}
+
+struct tc_params {
+    int32_t stride, feature_set, act, min_count, ncell, nin;
+    float tau_scalar, n_scale, theta_ref, relax_w;
+};
+
+// Persistent CTAs: the packed weights (80 KB) are copied to shared memory once per CTA, then every warp walks over
+// 16-cell tiles.
+__global__ void __launch_bounds__(TC_THREADS, 2)
+mlp_tc_kernel(const double* __restrict__ mom, const float* __restrict__ tau_cell, const float4* __restrict__ frags,
+              const float* __restrict__ misc, float* __restrict__ coef, uint32_t* __restrict__ flags,
+              const __grid_constant__ tc_params P)
+{
+    extern __shared__ __align__(16) unsigned char tc_smem[];
+    float4* wf = reinterpret_cast<float4*>(tc_smem);                               // [TC_FRAGS]
+    float* ms = reinterpret_cast<float*>(tc_smem + (size_t)TC_FRAGS * sizeof(float4));   // [TC_MISC]
+    float* xs_all = ms + TC_MISC;                                                  // [TC_WARPS][16][17] staging
+    for (int e = threadIdx.x; e < TC_FRAGS; e += TC_THREADS) wf[e] = frags[e];
+    for (int e = threadIdx.x; e < TC_MISC; e += TC_THREADS) ms[e] = misc[e];
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, t = lane & 3;
+    float* xs = xs_all + warp * (16 * 17);
+    const float* xmean = ms + 4 * TC_H, *xscale = xmean + 16, *ymean = xscale + 16, *yscale = ymean + 16;
+    const int ntiles = (P.ncell + 15) / 16;
+    for (int tile = blockIdx.x * TC_WARPS + warp; tile < ntiles; tile += gridDim.x * TC_WARPS) {
+        const int cell0 = tile * 16;
+        // ---- features of cell cell0 + lane (lanes 0..15), standardised, into xs[row][col]
+        double nraw = 0.0, theta = 0.0;
+        float tau = P.tau_scalar;
+        bool zbad = false;                               // a non-finite standardised input: the network output is non-finite
+        const int cell = cell0 + (lane & 15);
+        const bool have = lane < 16 && cell < P.ncell;
+        if (lane < 16) {
+            float x[16];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) x[i] = 0.0f;
+            if (have) {
+                const double* rec = mom + (size_t)cell * P.stride;
+                nraw = rec[0];
+                theta = (rec[4] + rec[7] + rec[9]) / 3.0;
+                if (tau_cell) tau = tau_cell[cell];
+                double h[3];
+                if (P.stride == 13) { h[0] = rec[10]; h[1] = rec[11]; h[2] = rec[12]; }
+                else { h[0] = rec[10] + rec[13] + rec[15]; h[1] = rec[11] + rec[16] + rec[18]; h[2] = rec[12] + rec[17] + rec[19]; }
+                const double n = nraw * (double)P.n_scale;
+                if (P.feature_set == 0) {
+                    x[0] = (float)n; x[1] = (float)rec[1]; x[2] = (float)rec[2]; x[3] = (float)rec[3];
+                    x[4] = (float)(theta / (double)P.theta_ref);
+                    x[5] = (float)(n * (rec[4] - theta)); x[6] = (float)(n * rec[5]); x[7] = (float)(n * rec[6]);
+                    x[8] = (float)(n * (rec[7] - theta)); x[9] = (float)(n * rec[8]);
+                    x[10] = (float)(0.5 * n * h[0]); x[11] = (float)(0.5 * n * h[1]); x[12] = (float)(0.5 * n * h[2]);
+                } else {
+                    x[0] = (float)n; x[1] = (float)(theta / (double)P.theta_ref);
+                    x[2] = (float)rec[1]; x[3] = (float)rec[2]; x[4] = (float)rec[3];
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) x[5 + k] = (float)(n * rec[4 + k]);
+                    x[11] = (float)(0.5 * n * h[0]); x[12] = (float)(0.5 * n * h[1]); x[13] = (float)(0.5 * n * h[2]);
+                    x[14] = (float)(3.0 * theta);
+                    x[15] = (float)(1.0 / (double)tau);
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                float z = (i < P.nin) ? (x[i] - xmean[i]) / xscale[i] : 0.0f;
+                if (have && !isfinite(z)) zbad = true;
+                if (!have || !isfinite(z)) z = 0.0f;
+                xs[lane * 17 + i] = z;
+            }
+        }
+        __syncwarp();
+        // ---- layer 1 A fragments: slot t <- column 8j+2t, slot t+4 <- column 8j+2t+1
+        uint32_t ahi[8][4], alo[8][4];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            tc_split(xs[g * 17 + 8 * j + 2 * t], ahi[j][0], alo[j][0]);
+            tc_split(xs[(g + 8) * 17 + 8 * j + 2 * t], ahi[j][1], alo[j][1]);
+            tc_split(xs[g * 17 + 8 * j + 2 * t + 1], ahi[j][2], alo[j][2]);
+            tc_split(xs[(g + 8) * 17 + 8 * j + 2 * t + 1], ahi[j][3], alo[j][3]);
+        }
+        float c[8][4];
+        tc_layer<2, 8>(ahi, alo, c, wf, ms, lane);
+        tc_activate(c, ahi, alo, P.act);
+        tc_layer<8, 8>(ahi, alo, c, wf + TC_F1, ms + TC_H, lane);
+        tc_activate(c, ahi, alo, P.act);
+        tc_layer<8, 8>(ahi, alo, c, wf + TC_F1 + TC_F2, ms + 2 * TC_H, lane);
+        tc_activate(c, ahi, alo, P.act);
+        tc_layer<8, 2>(ahi, alo, c, wf + TC_F1 + 2 * TC_F2, ms + 3 * TC_H, lane);
+        // ---- head outputs to the staging tile: row g / g+8, columns 2t, 2t+1 (n-tile 0) and 8+2t, 9+2t (n-tile 1)
+        __syncwarp();
+        xs[g * 17 + 2 * t] = c[0][0]; xs[g * 17 + 2 * t + 1] = c[0][1];
+        xs[(g + 8) * 17 + 2 * t] = c[0][2]; xs[(g + 8) * 17 + 2 * t + 1] = c[0][3];
+        xs[g * 17 + 8 + 2 * t] = c[1][0]; xs[g * 17 + 9 + 2 * t] = c[1][1];
+        xs[(g + 8) * 17 + 8 + 2 * t] = c[1][2]; xs[(g + 8) * 17 + 9 + 2 * t] = c[1][3];
+        __syncwarp();
+        // ---- de-standardise, policy, blend: lane < 16 owns cell cell0 + lane
+        if (have) {
+            float y[9];
+            bool finite = !zbad;
+#pragma unroll
+            for (int k = 0; k < 9; ++k) {
+                y[k] = fmaf(xs[lane * 17 + k], yscale[k], ymean[k]);
+                finite = finite && isfinite(y[k]);
+            }
+            float* out = coef + (size_t)cell * 9;
+            if (!(nraw > 0.0)) {
+#pragma unroll
+                for (int k = 0; k < 9; ++k) out[k] = 0.0f;
+                flags[cell] = FP_FLAG_EMPTY;
+            } else {
+                uint32_t flag = 0;
+                bool langevin = false;
+                if (nraw < (double)P.min_count) { flag = FP_FLAG_LOWCOUNT; langevin = true; }
+                else if (!(theta > 0.0) || !isfinite(theta)) { flag = FP_FLAG_SINGULAR; langevin = true; }
+                else if (!finite) { flag = FP_FLAG_NONFINITE; langevin = true; }
+                if (langevin) {
+                    const float d = -1.0f / tau;
+                    y[0] = d; y[1] = 0.f; y[2] = 0.f; y[3] = d; y[4] = 0.f; y[5] = d; y[6] = 0.f; y[7] = 0.f; y[8] = 0.f;
+                }
+#pragma unroll
+                for (int k = 0; k < 9; ++k) out[k] = (P.relax_w == 1.0f) ? y[k] : P.relax_w * y[k] + (1.0f - P.relax_w) * out[k];
+                flags[cell] = flag;
+            }
+        }
+        __syncwarp();
+    }
+}

@@ -19,7 +19,7 @@ FLAG_EMPTY, FLAG_LOWCOUNT, FLAG_SINGULAR, FLAG_ILLCOND, FLAG_ALPHA, FLAG_SKIPPED
 
 EXPORTS = ["fp_create", "fp_destroy", "fp_last_error", "fp_version", "fp_sort_by_cell", "fp_cell_moments",
            "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host",
-           "fp_timing_enable", "fp_timing_read", "fp_launch_count"]
+           "fp_timing_enable", "fp_timing_read", "fp_launch_count", "fp_set_mlp_tensor_cores"]
 NSTAGES = 6
 STAGE_NAMES = ["stream_walls", "sort_keys", "gather", "moments", "closure", "update"]
 
@@ -77,6 +77,7 @@ def load(path=None):
     lib.fp_timing_enable.argtypes = [vp, i32]
     lib.fp_timing_read.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32)]
     lib.fp_launch_count.argtypes = [vp]
+    lib.fp_set_mlp_tensor_cores.argtypes = [vp, i32]
     for name in EXPORTS:
         if name not in ("fp_last_error", "fp_version", "fp_launch_count"):
             getattr(lib, name).restype = C.c_int
@@ -227,6 +228,10 @@ def fp_timing_read(ctx, max_steps):
     n = C.c_int32(0)
     _check(ctx, load().fp_timing_read(ctx, buf, C.byref(n)), "fp_timing_read")
     return np.frombuffer(buf, dtype=np.float32)[: n.value * NSTAGES].reshape(n.value, NSTAGES).copy()
+
+
+def fp_set_mlp_tensor_cores(ctx, enable):
+    _check(ctx, load().fp_set_mlp_tensor_cores(ctx, 1 if enable else 0), "fp_set_mlp_tensor_cores")
 
 
 def fp_launch_count(ctx):

@@ -221,29 +221,34 @@ def test_closure_exact_langevin(gpu, wl):
 
 
 # ------------------------------------------------------------------------------------------------ a5 MLP surrogate
-@pytest.mark.parametrize("shape", ["13-64x3-silu", "13-64x3-relu", "16-32-relu", "13-7-5-silu", "16-256x4-relu"])
+@pytest.mark.parametrize("shape", ["13-64x3-silu", "13-64x3-relu", "16-64x3-silu", "16-32-relu", "13-7-5-silu", "16-256x4-relu"])
 @pytest.mark.parametrize("stride", [13, 29])
 def test_closure_mlp(gpu, wl, orc, shape, stride):
     import torch
     cfg, st = wl.ragged(nx=25, ny=16, seed=13, mean_ppc=60.0)
     s, cs = _sorted_case(orc, cfg, st)
     mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 1 if stride == 29 else 0)
-    dims, act, fs = {"13-64x3-silu": ((13, 64, 64, 64, 9), 0, 0), "13-64x3-relu": ((13, 64, 64, 64, 9), 1, 0),
+    dims, act, fs = {"13-64x3-silu": ((13, 64, 64, 64, 9), 0, 0), "13-64x3-relu": ((13, 64, 64, 64, 9), 1, 0), "16-64x3-silu": ((16, 64, 64, 64, 9), 0, 1),
                      "16-32-relu": ((16, 32, 9), 1, 1), "13-7-5-silu": ((13, 7, 5, 9), 0, 0),
                      "16-256x4-relu": ((16, 256, 256, 256, 256, 9), 1, 1)}[shape]
     mlp = wl.xavier_mlp(dims=dims, seed=0, act=act, feature_set=fs, n_scale=1.0 / 60.0, tau=cfg["tau"], bias_scale=0.1)
     tau = np.random.default_rng(3).uniform(0.4, 2.0, size=mom.shape[0]).astype(np.float32)
     ctx = gpu.Context(cfg)
     dm = gpu.Mlp(mlp)
-    for relax_w in (1.0, 0.2):
-        old = np.random.default_rng(8).normal(size=(mom.shape[0], 9)).astype(np.float32)
-        ref, rflags = orc.closure_mlp(mom, mlp, tau, min_count=cfg["min_count_mlp"], relax_w=relax_w, coef_old=old)
-        coef, flags = ctx.closure_mlp(torch.from_numpy(mom).cuda(), dm, torch.from_numpy(tau).cuda(), relax_w,
-                                      coef=torch.from_numpy(old.copy()).cuda())
-        coef, flags = coef.cpu().numpy(), flags.cpu().numpy().view(np.uint32)
-        assert np.array_equal(flags, rflags)
-        r = coef_ratio(coef, ref, tau, _theta(mom), 1e-5, mask=(rflags & orc.FLAG_EMPTY) == 0)
-        print("closure_mlp %s stride %d w %.1f: worst err/allowed %.3g" % (shape, stride, relax_w, r))
-        assert r <= 1.0
-        assert np.isfinite(coef).all()
+    # the benchmark shape runs on the tensor cores by default (3xTF32: ~1e-5 of the output scale; north_star allows
+    # 3e-3 for TF32); the plain fp32 kernel must meet 1e-5 for every shape, so it is checked as well
+    variants = [("fp32", False, 1e-5)] + ([("tf32x3", True, 3e-5)] if shape.startswith(("13-64x3", "16-64x3")) else [])
+    for vname, tc, tol in variants:
+      gpu.fp_set_mlp_tensor_cores(ctx.h, tc)
+      for relax_w in (1.0, 0.2):
+          old = np.random.default_rng(8).normal(size=(mom.shape[0], 9)).astype(np.float32)
+          ref, rflags = orc.closure_mlp(mom, mlp, tau, min_count=cfg["min_count_mlp"], relax_w=relax_w, coef_old=old)
+          coef, flags = ctx.closure_mlp(torch.from_numpy(mom).cuda(), dm, torch.from_numpy(tau).cuda(), relax_w,
+                                        coef=torch.from_numpy(old.copy()).cuda())
+          coef, flags = coef.cpu().numpy(), flags.cpu().numpy().view(np.uint32)
+          assert np.array_equal(flags, rflags)
+          r = coef_ratio(coef, ref, tau, _theta(mom), tol, mask=(rflags & orc.FLAG_EMPTY) == 0)
+          print("closure_mlp %s [%s] stride %d w %.1f: worst err/allowed %.3g (tol %.0e)" % (shape, vname, stride, relax_w, r, tol))
+          assert r <= 1.0
+          assert np.isfinite(coef).all()
     ctx.close()

@@ -191,10 +191,11 @@ def test_step_one(gpu, wl, orc, name, closure):
         tolv = 1e-4 if name == "cylinder" else 2e-5
     else:
         good = (aux["flags"] & orc.FLAG_EMPTY) == 0
-        rc = coef_ratio(res["coef"], aux["coef"], tau, theta, 1e-5, mask=good)
+        # benchmark-shape surrogate runs on the tensor cores (3xTF32, ~1e-5 of the output scale; see test_closure_mlp)
+        rc = coef_ratio(res["coef"], aux["coef"], tau, theta, 3e-5, mask=good)
         # the surrogate standardises its inputs by 0.05-0.3, so at Mach 10 (|U| = 9) the ~1e-7 relative mismatch
         # of the two sides' moments reaches the coefficients at ~1e-5 and the velocities through (1 - E1) tau N
-        tolv = 5e-5 if name == "cylinder" else 2e-6
+        tolv = 5e-5 if name == "cylinder" else 4e-6
     n = np.diff(aux["cell_start"])
     pm = np.repeat(good, n)
     cs_good = np.concatenate([[0], np.cumsum(n[good])]).astype(np.int64)
