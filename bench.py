@@ -34,8 +34,8 @@ UNIT = "particle-steps/s"
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="fpcl", choices=["fpcl", "reference"])
     ap.add_argument("--closure", default="exact", choices=["exact", "mlp"])
     ap.add_argument("--settle", type=int, default=200, help="untimed steps that relax the initial uniform counts")
@@ -250,22 +250,18 @@ def main():
         run_reference(args)
         return
     import torch
-    import torch.distributed as dist
-    from paper_2606_15622_b200 import fpcl, workloads
+    from paper_2606_15622_b200 import dist as D, fpcl, workloads
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local = D.world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    D.init("nccl", torch.device("cuda", local))
     hbm_peak, peak_src = peaks()
     closure = 0 if args.closure == "exact" else 1
 
     # independent replica per rank: same shape, different seed (weak scaling)
-    cfg, st, wname = workload(args, seed=3 + rank)
+    cfg, st, wname = workload(args, seed=D.replica_seed(3, rank))
     np_ = st["x"].shape[0]
     ncell = cfg["nx"] * cfg["ny"]
     mlp_host = workloads.xavier_mlp(n_scale=0.01, tau=cfg["tau"])
@@ -283,8 +279,7 @@ def main():
     settled = fpcl.to_host(a)                     # host copy of the settled ensemble: e2e and oracle input
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        D.barrier()
         torch.cuda.synchronize()
 
     # ---- timed region: K fp_step calls, device-resident
@@ -310,11 +305,8 @@ def main():
     launches = fpcl.fp_launch_count(ctx.h) - l0
     stage_ms = fpcl.fp_timing_read(ctx.h, args.steps)
     fpcl.fp_timing_enable(ctx.h, 0)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
-    value = world * np_ * args.steps / (ms_total * 1e-3)
+    ms_total = D.max_over_ranks(ms_total, "cuda")
+    value = D.aggregate_throughput(np_, args.steps, ms_total, world)
     flags_host = out["flags"].cpu().numpy().view(np.uint32)
 
     # ---- end to end through fp_step_host: pinned host buffers, H2D + D2H inside the timed region
@@ -333,10 +325,7 @@ def main():
                       h_cell_start=hs)
     barrier()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * np_ * e2e_steps / float(t.item())
+    e2e_value = D.aggregate_throughput(np_, e2e_steps, 1e3 * D.max_over_ranks(e2e_s, "cuda"), world)
     h2d = 24 * np_
     d2h = 24 * np_ + ncell * (36 + 4) + (ncell + 1) * 4
 
@@ -399,8 +388,7 @@ def main():
         line.update(extras)
         print(json.dumps(line, default=float))
     ctx.close()
-    if world > 1:
-        dist.destroy_process_group()
+    D.shutdown()
 
 
 if __name__ == "__main__":

@@ -314,3 +314,50 @@ def test_full_size_cavity(gpu, wl, orc):
     for k in ("vx", "vy", "vz"):
         assert np.isfinite(got[k]).all()
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ fallback paths
+def test_unstaged_paths(gpu, wl, orc):
+    """Per-warp staging needs 16-byte aligned arrays and cells that fit the warp's buffer.  Unaligned views and a
+    cell of several thousand particles must take the global-memory path and still match the oracle."""
+    import torch
+    cfg, st = wl.ragged(nx=12, ny=9, seed=31, mean_ppc=70.0)
+    # one huge cell: move 4000 extra particles into cell 17
+    rng = np.random.default_rng(1)
+    extra = 4000
+    ex = {k: np.empty(extra, np.float32) for k in ("x", "y", "vx", "vy", "vz")}
+    ex["x"][:] = (17 % 12 + rng.uniform(0.1, 0.9, extra)) / 12
+    ex["y"][:] = (17 // 12 + rng.uniform(0.1, 0.9, extra)) / 9
+    for k in ("vx", "vy", "vz"):
+        ex[k][:] = rng.normal(0.2, 0.9, extra)
+    st = {k: np.concatenate([st[k], ex[k]]) for k in ("x", "y", "vx", "vy", "vz")}
+    st["pid"] = np.arange(st["x"].shape[0], dtype=np.uint32)
+    cfg = dict(cfg, max_particles=int(st["x"].shape[0]) + 8)
+    s, cs, _ = orc.sort_by_cell(st, cfg)
+    n = s["x"].shape[0]
+    ctx = gpu.Context(cfg)
+    for off in (0, 1):          # off = 1: every array starts 4 bytes past a 16-byte boundary
+        def dev(a, dt):
+            buf = torch.empty(n + 4, dtype=dt, device="cuda")
+            v = buf[off:off + n]
+            v.copy_(torch.from_numpy(a.view(np.int32) if a.dtype == np.uint32 else a))
+            return v
+        vx, vy, vz = dev(s["vx"], torch.float32), dev(s["vy"], torch.float32), dev(s["vz"], torch.float32)
+        pid = dev(s["pid"], torch.int32)
+        csd = torch.from_numpy(cs).cuda()
+        for mode in (0, 1):
+            ref = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, mode)
+            mom = ctx.cell_moments(vx, vy, vz, csd, mode)
+            r = moment_ratio(mom.cpu().numpy(), ref, absmom=abs_moments(s["vx"], s["vy"], s["vz"], cs, ref))
+            assert r <= 1.0, (off, mode, r)
+        mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 1)
+        coef, flags, _ = orc.closure_exact(mom, cfg["tau"], cfg["eps2_scale"], cfg["min_count"])
+        c32 = coef.astype(np.float32)
+        rvx, rvy, rvz, rfl = orc.velocity_update(s["vx"], s["vy"], s["vz"], s["pid"], cs, mom, c32, cfg["tau"], cfg, 11, flags)
+        fl = torch.from_numpy(flags.view(np.int32).copy()).cuda()
+        ctx.velocity_update(vx, vy, vz, pid, csd, torch.from_numpy(mom).cuda(), torch.from_numpy(c32).cuda(), 11, fl)
+        rv = velocity_ratio((vx.cpu().numpy(), vy.cpu().numpy(), vz.cpu().numpy()), (rvx, rvy, rvz), cs, _theta(mom))
+        print("unstaged offset %d: update worst err/allowed %.3f" % (off, rv))
+        assert rv <= 1.0
+        assert np.array_equal(fl.cpu().numpy().view(np.uint32), rfl)
+    ctx.close()
