@@ -66,7 +66,7 @@ def workload(args, seed):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -77,7 +77,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -342,8 +342,13 @@ def main():
     # dominant single kernel of the step (sort_keys is six launches; the others are one kernel each)
     single = {n: stages[n] for n in ("stream_walls", "gather", "moments", "closure", "update")}
     dom = max(single, key=lambda n: single[n]["ms"])
+    # DRAM traffic per launch from the committed ncu --set full capture (profiles/r01_ncu_full_v2.md, C3), bytes;
+    # the in-place update's writes are still in L2 when its kernel ends, so its figure is mostly reads
+    ncu_traffic = {"update": 70.3e6 + 10.9e6, "moments": 48.4e6, "gather": 204.1e6, "stream_walls": 88.3e6,
+                   "closure": 9.3e6 if closure == 0 else 4.3e6}
     roofline = {"kernel": dom, "bound": "hbm", "achieved": single[dom]["GBps_algorithmic"], "peak": hbm_peak,
-                "unit": "GB/s", "frac": single[dom]["frac_of_hbm_peak"], "traffic": None,
+                "unit": "GB/s", "frac": single[dom]["frac_of_hbm_peak"],
+                "traffic": ncu_traffic.get(dom) if not args.small else None,
                 "peak_source": peak_src, "timing": "CUDA events inside fp_step, median over the timed steps (L2-warm)"}
 
     extras = {}

@@ -92,18 +92,25 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t mask = (uint32_t)bins - 1u;
     for (int b = threadIdx.x; b < bins * SORT_WARPS; b += SORT_THREADS) (&cnt[0][0])[(b / bins) * SORT_MAX_BINS + (b % bins)] = 0;
-    // exclusive scan of the digit totals (bins <= 512) by warp 0, two elements per pass
-    if (warp == 0) {
-        uint32_t carry = 0;
-        for (int b0 = 0; b0 < bins; b0 += 32) {
-            const int b = b0 + lane;
-            const uint32_t v = (b < bins) ? bin_total[b] : 0u;
-            uint32_t s = v;
+    // exclusive scan of the digit totals (bins <= 512 = 8 warps x 32 lanes x 2 consecutive bins): every thread fetches
+    // its two totals and its two tile offsets at once (one global latency), warps scan, warp totals go through smem
+    {
+        __shared__ uint32_t wtot[SORT_WARPS];
+        const int b0 = 2 * (int)threadIdx.x, b1 = b0 + 1;
+        const uint32_t v0 = (b0 < bins) ? bin_total[b0] : 0u, v1 = (b1 < bins) ? bin_total[b1] : 0u;
+        const uint32_t h0 = (b0 < bins) ? block_hist[(size_t)b0 * nblocks + blockIdx.x] : 0u;
+        const uint32_t h1 = (b1 < bins) ? block_hist[(size_t)b1 * nblocks + blockIdx.x] : 0u;
+        uint32_t incl = v0 + v1;
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, s, d); if (lane >= d) s += t; }
-            if (b < bins) bin_base[b] = carry + s - v + block_hist[(size_t)b * nblocks + blockIdx.x];
-            carry += __shfl_sync(0xffffffffu, s, 31);
-        }
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
+        if (lane == 31) wtot[warp] = incl;
+        __syncthreads();
+        uint32_t wb = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) if (w < warp) wb += wtot[w];
+        const uint32_t e = wb + incl - (v0 + v1);
+        if (b0 < bins) bin_base[b0] = e + h0;
+        if (b1 < bins) bin_base[b1] = e + v0 + h1;
     }
     __syncthreads();
     const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS);
@@ -123,7 +130,7 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
         const uint32_t act = __ballot_sync(0xffffffffu, valid[i]);
         uint32_t r = 0;
         if (valid[i]) {
-            const uint32_t peers = __match_any_sync(act, d);
+            const uint32_t peers = __match_any_sync(act, d);   // (a ballot-per-bit search measured slower: 111 vs 99 us)
             const int leader = __ffs(peers) - 1;
             const uint32_t before = __popc(peers & ((1u << lane) - 1u));
             uint32_t c = 0;
