@@ -134,13 +134,13 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
     const int32_t stride = mode ? 29 : 13;
     if ((rc = fp_cell_moments(ctx, np, vx_b, vy_b, vz_b, cell_start, mode, mom, stream)) != FP_OK) return rc;
     fp_mark(ctx, 4, st);
-    // a4 | a5
-    if (closure == 0) rc = fp_closure_exact(ctx, mom, tau_use, coef, flags, nullptr, stream);
-    else              rc = fp_closure_mlp(ctx, mom, stride, tau_use, h_mlp, relax_w, coef, flags, stream);
+    // a4 | a5; the closure kernel also writes the per-cell constants of a6 (no separate prep launch)
+    if (closure == 0) rc = fpi_closure_exact(ctx, mom, tau_use, coef, flags, nullptr, true, st);
+    else              rc = fpi_closure_mlp(ctx, mom, stride, tau_use, h_mlp, relax_w, coef, flags, true, st);
     if (rc != FP_OK) return rc;
     fp_mark(ctx, 5, st);
     // a6
-    rc = fpi_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, st);
+    rc = fpi_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, true, st);
     fp_mark(ctx, 6, st);
     return rc;
 }

@@ -13,6 +13,7 @@
 // 9x10 system to shared memory as [entry][thread] (conflict free, dynamic row index = free pivoting without register
 // selects) and eliminates in place.  The system never touches HBM: 232 B/cell in, 40 B/cell out.
 #include "tiles.cuh"
+#include "upd_prep.cuh"
 
 #define CE_TPB 64
 
@@ -70,7 +71,7 @@ __device__ __forceinline__ void ce_build_row(const ce_scaled& m, double (&a)[10]
 __global__ void __launch_bounds__(CE_TPB)
 closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ tau_cell, float tau_scalar,
                      float eps2_scale, int32_t min_count, int32_t ncell, float* __restrict__ coef,
-                     uint32_t* __restrict__ flags, double* __restrict__ kappa_est)
+                     uint32_t* __restrict__ flags, double* __restrict__ kappa_est, float* __restrict__ cellc, float dt)
 {
     extern __shared__ double ce_sm[];
     double* recs = ce_sm;                        // [CE_TPB * 29] staged records
@@ -87,16 +88,16 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
     const double tau = (double)(tau_cell ? tau_cell[cell] : tau_scalar);
     const double theta = (rec[4] + rec[7] + rec[9]) / 3.0;
     const bool theta_ok = (theta > 0.0) && isfinite(theta);
-    float* out = coef + (size_t)cell * 9;
+    float cf[9];                                 // the coefficients as stored
+    uint32_t flag = 0;
+    double kap = 0.0;
     // ---- policy for cells that are not solved (R3-c)
     if (!(n > 0.0) || n < (double)min_count || !theta_ok) {
         const bool empty = !(n > 0.0);
         const float d = empty ? 0.0f : (float)(-1.0 / tau);
-        out[0] = d; out[1] = 0.f; out[2] = 0.f; out[3] = d; out[4] = 0.f; out[5] = d; out[6] = 0.f; out[7] = 0.f; out[8] = 0.f;
-        flags[cell] = empty ? FP_FLAG_EMPTY : (n < (double)min_count ? FP_FLAG_LOWCOUNT : FP_FLAG_SINGULAR);
-        if (kappa_est) kappa_est[cell] = 0.0;
-        return;
-    }
+        cf[0] = d; cf[1] = 0.f; cf[2] = 0.f; cf[3] = d; cf[4] = 0.f; cf[5] = d; cf[6] = 0.f; cf[7] = 0.f; cf[8] = 0.f;
+        flag = empty ? FP_FLAG_EMPTY : (n < (double)min_count ? FP_FLAG_LOWCOUNT : FP_FLAG_SINGULAR);
+    } else {
 #define CE_A(i, j) As[((i) * 10 + (j)) * CE_TPB + tid]
     double anorm = 0.0, bmax = 0.0;
     {
@@ -184,11 +185,9 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
     double ymax = 0.0;
 #pragma unroll
     for (int k = 0; k < 9; ++k) { finite = finite && isfinite(y[k]); ymax = fmax(ymax, fabs(y[k])); }
-    uint32_t flag = 0;
-    double kap = 0.0;
     if (!(minpiv >= 1e-14) || !finite) {
         const float d = (float)(-1.0 / tau);
-        out[0] = d; out[1] = 0.f; out[2] = 0.f; out[3] = d; out[4] = 0.f; out[5] = d; out[6] = 0.f; out[7] = 0.f; out[8] = 0.f;
+        cf[0] = d; cf[1] = 0.f; cf[2] = 0.f; cf[3] = d; cf[4] = 0.f; cf[5] = d; cf[6] = 0.f; cf[7] = 0.f; cf[8] = 0.f;
         flag = FP_FLAG_SINGULAR;
     } else {
         const double k1 = bmax > 0.0 ? anorm * ymax / bmax : 0.0;
@@ -196,19 +195,23 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
         if (!(kap < 1e8)) flag = FP_FLAG_ILLCOND;
         const double ic = 1.0 / tau, ig = 1.0 / (tau * sqrt(theta));
 #pragma unroll
-        for (int k = 0; k < 6; ++k) out[k] = (float)(y[k] * ic);
+        for (int k = 0; k < 6; ++k) cf[k] = (float)(y[k] * ic);
 #pragma unroll
-        for (int k = 6; k < 9; ++k) out[k] = (float)(y[k] * ig);
+        for (int k = 6; k < 9; ++k) cf[k] = (float)(y[k] * ig);
     }
+    }   // solved cells
+    float* out = coef + (size_t)cell * 9;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) out[k] = cf[k];
+    // inside fp_step the velocity update follows: hand it its per-cell constants now (upd_prep.cuh)
+    if (cellc) flag |= upd_prep_cell(rec, 29, cf, tau, dt, eps2_scale, cellc + (size_t)cell * UPD_NC);
     flags[cell] = flag;
     if (kappa_est) kappa_est[cell] = kap;
 }
 
-extern "C" int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell, float* coef,
-                                uint32_t* flags, double* kappa_est, void* stream)
+int fpi_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell, float* coef, uint32_t* flags,
+                      double* kappa_est, bool with_update_constants, cudaStream_t stream)
 {
-    if (!ctx) return FP_ERR_ARG;
-    if (!mom_full || !coef || !flags) return fp_fail(ctx, FP_ERR_ARG, "fp_closure_exact: null pointer");
     const int32_t ncell = ctx->ncell;
     const int blocks = fp_div_up(ncell, CE_TPB);
     const size_t smem = (size_t)CE_TPB * (29 + 90) * sizeof(double);
@@ -217,9 +220,18 @@ extern "C" int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float
         FP_CUDA_OK(ctx, cudaFuncSetAttribute(closure_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    closure_exact_kernel<<<blocks, CE_TPB, smem, (cudaStream_t)stream>>>(mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
-                                                                       ctx->p.min_count, ncell, coef, flags, kappa_est);
+    closure_exact_kernel<<<blocks, CE_TPB, smem, stream>>>(mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
+                                                                       ctx->p.min_count, ncell, coef, flags, kappa_est,
+                                                                       with_update_constants ? ctx->cellc : nullptr, ctx->p.dt);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
     return FP_OK;
+}
+
+extern "C" int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell, float* coef,
+                                uint32_t* flags, double* kappa_est, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    if (!mom_full || !coef || !flags) return fp_fail(ctx, FP_ERR_ARG, "fp_closure_exact: null pointer");
+    return fpi_closure_exact(ctx, mom_full, tau_cell, coef, flags, kappa_est, false, (cudaStream_t)stream);
 }

@@ -9,6 +9,7 @@
 // inputs, so one activation load and two broadcast 128-bit weight loads feed 8 FMAs.  Plain fp32 FMA pipe
 // (tolerance 1e-5); no tensor cores in this kernel.
 #include "common.cuh"
+#include "upd_prep.cuh"
 
 #define MLP_OB 8
 
@@ -55,7 +56,8 @@ template <int CB>
 __global__ void __launch_bounds__(CB)
 mlp_kernel(const double* __restrict__ mom, int32_t stride, const float* __restrict__ tau_cell, float tau_scalar,
            const float* __restrict__ blob, const __grid_constant__ mlp_desc D, int32_t w_in_smem, int32_t min_count,
-           float relax_w, int32_t ncell, float* __restrict__ coef, uint32_t* __restrict__ flags)
+           float relax_w, int32_t ncell, float* __restrict__ coef, uint32_t* __restrict__ flags,
+           float* __restrict__ cellc, float dt, float eps2_scale)
 {
     extern __shared__ __align__(16) float smem[];
     float* wsm = smem;
@@ -145,23 +147,29 @@ mlp_kernel(const double* __restrict__ mom, int32_t stride, const float* __restri
         finite = finite && isfinite(y[k]);
     }
     uint32_t flag = 0;
-    bool langevin = false;
     float* out = coef + (size_t)cell * 9;
     if (!(nraw > 0.0)) {
 #pragma unroll
-        for (int k = 0; k < 9; ++k) out[k] = 0.0f;
-        flags[cell] = FP_FLAG_EMPTY;
-        return;
-    }
-    if (nraw < (double)min_count) { flag = FP_FLAG_LOWCOUNT; langevin = true; }
-    else if (!(theta > 0.0) || !isfinite(theta)) { flag = FP_FLAG_SINGULAR; langevin = true; }
-    else if (!finite) { flag = FP_FLAG_NONFINITE; langevin = true; }
-    if (langevin) {
-        const float d = -1.0f / tau;
-        y[0] = d; y[1] = 0.f; y[2] = 0.f; y[3] = d; y[4] = 0.f; y[5] = d; y[6] = 0.f; y[7] = 0.f; y[8] = 0.f;
+        for (int k = 0; k < 9; ++k) y[k] = 0.0f;
+        flag = FP_FLAG_EMPTY;
+    } else {
+        bool langevin = false;
+        if (nraw < (double)min_count) { flag = FP_FLAG_LOWCOUNT; langevin = true; }
+        else if (!(theta > 0.0) || !isfinite(theta)) { flag = FP_FLAG_SINGULAR; langevin = true; }
+        else if (!finite) { flag = FP_FLAG_NONFINITE; langevin = true; }
+        if (langevin) {
+            const float d = -1.0f / tau;
+            y[0] = d; y[1] = 0.f; y[2] = 0.f; y[3] = d; y[4] = 0.f; y[5] = d; y[6] = 0.f; y[7] = 0.f; y[8] = 0.f;
+        }
+        if (relax_w != 1.0f) {
+#pragma unroll
+            for (int k = 0; k < 9; ++k) y[k] = relax_w * y[k] + (1.0f - relax_w) * out[k];
+        }
     }
 #pragma unroll
-    for (int k = 0; k < 9; ++k) out[k] = (relax_w == 1.0f) ? y[k] : relax_w * y[k] + (1.0f - relax_w) * out[k];
+    for (int k = 0; k < 9; ++k) out[k] = y[k];
+    // inside fp_step the velocity update follows: hand it its per-cell constants now (upd_prep.cuh)
+    if (cellc) flag |= upd_prep_cell(rec, stride, y, (double)tau, dt, eps2_scale, cellc + (size_t)cell * UPD_NC);
     flags[cell] = flag;
 }
 
@@ -176,6 +184,13 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
                               const fp_mlp* h_mlp, float relax_w, float* coef, uint32_t* flags, void* stream)
 {
     if (!ctx) return FP_ERR_ARG;
+    return fpi_closure_mlp(ctx, mom, mom_stride, tau_cell, h_mlp, relax_w, coef, flags, false, (cudaStream_t)stream);
+}
+
+int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell, const fp_mlp* h_mlp,
+                    float relax_w, float* coef, uint32_t* flags, bool with_update_constants, cudaStream_t st)
+{
+    float* cellc = with_update_constants ? ctx->cellc : nullptr;
     if (!mom || !h_mlp || !coef || !flags || (mom_stride != 13 && mom_stride != 29))
         return fp_fail(ctx, FP_ERR_ARG, "fp_closure_mlp: null pointer or bad mom_stride");
     const fp_mlp& M = *h_mlp;
@@ -210,7 +225,6 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
     D.blob_floats = off; D.maxw = maxw;
     D.act = M.act; D.feature_set = M.feature_set; D.n_scale = M.n_scale; D.theta_ref = M.theta_ref;
     S.x_mean = M.x_mean; S.x_scale = M.x_scale; S.y_mean = M.y_mean; S.y_scale = M.y_scale;
-    cudaStream_t st = (cudaStream_t)stream;
     fp_mlp_dev& C = ctx->mlp;
     // ---- tensor-core path for the benchmark shape [13|16]-64-64-64-9
     if (!ctx->mlp_force_fp32 && M.n_layers == 4 && D.dims[1] == TC_H && D.dims[2] == TC_H && D.dims[3] == TC_H) {
@@ -223,6 +237,7 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
         P.stride = mom_stride; P.feature_set = M.feature_set; P.act = M.act; P.min_count = ctx->p.min_count_mlp;
         P.ncell = ctx->ncell; P.nin = D.dims[0]; P.tau_scalar = ctx->p.tau; P.n_scale = M.n_scale;
         P.theta_ref = M.theta_ref; P.relax_w = relax_w;
+        P.dt = ctx->p.dt; P.eps2_scale = ctx->p.eps2_scale; P.cellc = cellc;
         const size_t smem = fbytes + (size_t)TC_WARPS * 16 * 17 * sizeof(float);
         static int occ = 0;
         if (occ == 0) {
@@ -254,7 +269,8 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
         const size_t smem = abytes + (w_in_smem ? wbytes : 0);
         FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_kernel<CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         mlp_kernel<CB><<<fp_div_up(ncell, CB), CB, smem, st>>>(mom, mom_stride, tau_cell, ctx->p.tau, C.blob, D, w_in_smem,
-                                                             ctx->p.min_count_mlp, relax_w, ncell, coef, flags);
+                                                             ctx->p.min_count_mlp, relax_w, ncell, coef, flags, cellc,
+                                                             ctx->p.dt, ctx->p.eps2_scale);
     } else if (maxw <= 512) {
         constexpr int CB = 32;
         const size_t abytes = (size_t)2 * maxw * CB * sizeof(float);
@@ -262,7 +278,8 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
         const size_t smem = abytes + (w_in_smem ? wbytes : 0);
         FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_kernel<CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         mlp_kernel<CB><<<fp_div_up(ncell, CB), CB, smem, st>>>(mom, mom_stride, tau_cell, ctx->p.tau, C.blob, D, w_in_smem,
-                                                             ctx->p.min_count_mlp, relax_w, ncell, coef, flags);
+                                                             ctx->p.min_count_mlp, relax_w, ncell, coef, flags, cellc,
+                                                             ctx->p.dt, ctx->p.eps2_scale);
     } else {
         return fp_fail(ctx, FP_ERR_UNSUPPORTED, "fp_closure_mlp: hidden width > 512 is not supported");
     }

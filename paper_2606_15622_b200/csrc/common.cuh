@@ -104,6 +104,11 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
 int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
                      const uint32_t* pid, uint64_t step, uint32_t* keys_out /* nullable */, cudaStream_t st);
 int fpi_tau_from_counts(fp_ctx* ctx, const int32_t* cell_start, float tau_ref_n, float* tau_cell, cudaStream_t st);
+// the closures; with_update_constants: also fill ctx->cellc for the velocity update that follows (upd_prep.cuh)
+int fpi_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell, float* coef, uint32_t* flags,
+                      double* kappa_est, bool with_update_constants, cudaStream_t st);
+int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell, const fp_mlp* h_mlp,
+                    float relax_w, float* coef, uint32_t* flags, bool with_update_constants, cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------------------
 // Device helpers

@@ -130,6 +130,8 @@ __device__ __forceinline__ void tc_activate(const float (&c)[8][4], uint32_t (&a
 struct tc_params {
     int32_t stride, feature_set, act, min_count, ncell, nin;
     float tau_scalar, n_scale, theta_ref, relax_w;
+    float dt, eps2_scale;
+    float* cellc;                 // non-null inside fp_step: also write the velocity update's per-cell constants
 };
 
 // Persistent CTAs: the packed weights (80 KB) are copied to shared memory once per CTA, then every warp walks over
@@ -231,12 +233,12 @@ mlp_tc_kernel(const double* __restrict__ mom, const float* __restrict__ tau_cell
                 finite = finite && isfinite(y[k]);
             }
             float* out = coef + (size_t)cell * 9;
+            uint32_t flag = 0;
             if (!(nraw > 0.0)) {
 #pragma unroll
-                for (int k = 0; k < 9; ++k) out[k] = 0.0f;
-                flags[cell] = FP_FLAG_EMPTY;
+                for (int k = 0; k < 9; ++k) y[k] = 0.0f;
+                flag = FP_FLAG_EMPTY;
             } else {
-                uint32_t flag = 0;
                 bool langevin = false;
                 if (nraw < (double)P.min_count) { flag = FP_FLAG_LOWCOUNT; langevin = true; }
                 else if (!(theta > 0.0) || !isfinite(theta)) { flag = FP_FLAG_SINGULAR; langevin = true; }
@@ -245,10 +247,18 @@ mlp_tc_kernel(const double* __restrict__ mom, const float* __restrict__ tau_cell
                     const float d = -1.0f / tau;
                     y[0] = d; y[1] = 0.f; y[2] = 0.f; y[3] = d; y[4] = 0.f; y[5] = d; y[6] = 0.f; y[7] = 0.f; y[8] = 0.f;
                 }
+                if (P.relax_w != 1.0f) {
 #pragma unroll
-                for (int k = 0; k < 9; ++k) out[k] = (P.relax_w == 1.0f) ? y[k] : P.relax_w * y[k] + (1.0f - P.relax_w) * out[k];
-                flags[cell] = flag;
+                    for (int k = 0; k < 9; ++k) y[k] = P.relax_w * y[k] + (1.0f - P.relax_w) * out[k];
+                }
             }
+#pragma unroll
+            for (int k = 0; k < 9; ++k) out[k] = y[k];
+            // inside fp_step the velocity update follows: hand it its per-cell constants now (upd_prep.cuh)
+            if (P.cellc)
+                flag |= upd_prep_cell(mom + (size_t)cell * P.stride, P.stride, y, (double)tau, P.dt, P.eps2_scale,
+                                      P.cellc + (size_t)cell * UPD_NC);
+            flags[cell] = flag;
         }
         __syncwarp();
     }

@@ -97,4 +97,4 @@ __device__ __forceinline__ fpw_range fpw_range_of(int32_t s0, int32_t s1, int64_
 
 int fpi_velocity_update(fp_ctx* ctx, int64_t np, float* vx, float* vy, float* vz, const uint32_t* pid,
                         const int32_t* cell_start, const double* mom, int32_t mom_stride, const float* coef,
-                        const float* tau_cell, uint64_t step, uint32_t* flags, cudaStream_t st);
+                        const float* tau_cell, uint64_t step, uint32_t* flags, bool prep_done, cudaStream_t st);
