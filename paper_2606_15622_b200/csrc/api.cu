@@ -57,10 +57,11 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && sms > 0) c->num_sms = sms;
     const size_t n = (size_t)(q.max_particles > 0 ? q.max_particles : 1);
     const size_t nblocks = (n + SORT_TILE - 1) / SORT_TILE;
-    c->block_hist_elems = 512 * nblocks;
+    c->block_hist_elems = 512 * nblocks;               // per table; two tables (even / odd radix pass)
     bool ok = cudaMalloc((void**)&c->key_a, n * 4) == cudaSuccess && cudaMalloc((void**)&c->key_b, n * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->idx_a, n * 4) == cudaSuccess && cudaMalloc((void**)&c->idx_b, n * 4) == cudaSuccess &&
-              cudaMalloc((void**)&c->block_hist, c->block_hist_elems * 4) == cudaSuccess &&
+              cudaMalloc((void**)&c->block_hist, 2 * c->block_hist_elems * 4) == cudaSuccess &&
+              cudaMemset(c->block_hist, 0, 2 * c->block_hist_elems * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->bin_total, 512 * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->cellc, (size_t)c->ncell * 28 * 4) == cudaSuccess;
     if (!ok) { fp_free_all(c); delete c; cudaGetLastError(); return FP_ERR_CUDA; }
@@ -118,10 +119,10 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
     struct step_guard { fp_ctx* c; ~step_guard() { if (c->t_in_step) { c->t_in_step = false; c->t_step += 1; } } } guard{ctx};
     fp_mark(ctx, 0, st);
     // a0 + a1 (+ cell keys of the streamed positions)
-    if ((rc = fpi_stream_walls(ctx, np, x_a, y_a, vx_a, vy_a, vz_a, pid_a, step, ctx->key_b, st)) != FP_OK) return rc;
+    if ((rc = fpi_stream_walls(ctx, np, x_a, y_a, vx_a, vy_a, vz_a, pid_a, step, ctx->key_b, true, st)) != FP_OK) return rc;
     fp_mark(ctx, 1, st);
     // a2 (records mark 2 between the key sort and the payload gather)
-    if ((rc = fpi_sort_with_keys(ctx, np, ctx->key_b, false, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b,
+    if ((rc = fpi_sort_with_keys(ctx, np, ctx->key_b, true, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b,
                                  cell_start, nullptr, st)) != FP_OK) return rc;
     fp_mark(ctx, 3, st);
     const float* tau_use = nullptr;

@@ -46,7 +46,8 @@ struct fp_ctx {
     int       device = 0, num_sms = FPCL_NUM_SMS_DEFAULT;
     // sort scratch (sized for max_particles)
     uint32_t *key_a = nullptr, *key_b = nullptr, *idx_a = nullptr, *idx_b = nullptr;
-    uint32_t *block_hist = nullptr;  // [bins][nblocks]
+    uint32_t *block_hist = nullptr;  // two tables [bins][nblocks]: even passes use the first, odd passes the second
+    bool      hist0_clean = true;    // the first table is all zero (what the stream kernel's fused histogram needs)
     uint32_t *bin_total = nullptr;   // [bins]
     size_t    block_hist_elems = 0;
     float    *cellc = nullptr;       // [ncell * 28] per-cell constants of the velocity update (update.cu)
@@ -102,7 +103,8 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
                        const uint32_t* pid, float* x_out, float* y_out, float* vx_out, float* vy_out,
                        float* vz_out, uint32_t* pid_out, int32_t* cell_start, uint32_t* perm, cudaStream_t st);
 int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
-                     const uint32_t* pid, uint64_t step, uint32_t* keys_out /* nullable */, cudaStream_t st);
+                     const uint32_t* pid, uint64_t step, uint32_t* keys_out /* nullable */,
+                     bool with_hist0 /* also the first pass's tile histograms, needs keys_out */, cudaStream_t st);
 int fpi_tau_from_counts(fp_ctx* ctx, const int32_t* cell_start, float tau_ref_n, float* tau_cell, cudaStream_t st);
 // the closures; with_update_constants: also fill ctx->cellc for the velocity update that follows (upd_prep.cuh)
 int fpi_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell, float* coef, uint32_t* flags,

@@ -54,10 +54,14 @@ hist_kernel(int64_t np, const uint32_t* __restrict__ keys, uint32_t* __restrict_
     for (int b = threadIdx.x; b < bins; b += SORT_THREADS) block_hist[(size_t)b * nblocks + blockIdx.x] = h[b];
 }
 
-// one block per digit value: exclusive scan of that digit's counts over tiles (in place) and the digit total
+// one block per digit value: exclusive scan of that digit's counts over tiles (in place) and the digit total;
+// also zeroes the same row of the other table
 __global__ void __launch_bounds__(256)
-scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_total, int nblocks)
+scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_total, int nblocks,
+                 uint32_t* __restrict__ other_table)
 {
+    // the other pass's table is free now: clear this digit's row for the reductions that fill it next
+    for (int i = threadIdx.x; i < nblocks; i += 256) other_table[(size_t)blockIdx.x * nblocks + i] = 0u;
     __shared__ uint32_t wsum[8];
     uint32_t* row = block_hist + (size_t)blockIdx.x * nblocks;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -80,12 +84,16 @@ scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_t
 
 // stable scatter of one tile.  Warp w owns items [w*256, (w+1)*256) of the tile in warp-striped order
 // (round i, lane l -> w*256 + i*32 + l), so (tile, warp, round, lane) order is input order.
+#ifndef SORT_SCATTER_MINB
+#define SORT_SCATTER_MINB 4                               // 64 registers: four tiles per SM hide the latency phases
+#endif
+__device__ __forceinline__ int dbits_of(int bins) { return 31 - __clz(bins); }
 template <bool FIRST_PASS>
-__global__ void __launch_bounds__(SORT_THREADS)
+__global__ void __launch_bounds__(SORT_THREADS, SORT_SCATTER_MINB)
 scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
                uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out,
                const uint32_t* __restrict__ block_hist, const uint32_t* __restrict__ bin_total, int nblocks,
-               int shift, int bins)
+               int shift, int bins, uint32_t* __restrict__ next_hist)
 {
     __shared__ uint32_t cnt[SORT_WARPS][SORT_MAX_BINS];   // per-warp running digit counts, then bases
     __shared__ uint32_t bin_base[SORT_MAX_BINS];          // global start of each digit value + this tile's offset
@@ -151,11 +159,20 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < SORT_ITEMS; ++i) {
+        uint32_t code = 0xffffffffu;               // (next digit, next tile) of this item
         if (valid[i]) {
             const uint32_t d = (key[i] >> shift) & mask;
             const uint32_t dst = bin_base[d] + cnt[warp][d] + rank[i];
             keys_out[dst] = key[i];
             idx_out[dst] = idx[i];
+            code = (((key[i] >> shift) >> dbits_of(bins)) & mask) << 20 | (dst / SORT_TILE);
+        }
+        // the next pass's tile histograms: the tile an item lands in is known here, so lanes that agree on
+        // (next digit, next tile) send one aggregated reduction to the (zeroed) table of the next pass
+        if (next_hist) {
+            const uint32_t peers = __match_any_sync(0xffffffffu, code);
+            if (valid[i] && lane == __ffs(peers) - 1)
+                atomicAdd(&next_hist[(size_t)(code >> 20) * nblocks + (code & 0xfffffu)], (uint32_t)__popc(peers));
         }
     }
 }
@@ -219,21 +236,25 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     uint32_t* iout = ctx->idx_a;
     for (int pass = 0; pass < passes; ++pass) {
         const int shift = pass * dbits;
-        if (!(pass == 0 && hist0_ready)) {
-            hist_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, kin, ctx->block_hist, nblocks, shift, bins);
+        uint32_t* table = ctx->block_hist + (size_t)(pass & 1) * ctx->block_hist_elems;
+        uint32_t* other = ctx->block_hist + (size_t)((pass + 1) & 1) * ctx->block_hist_elems;
+        if (pass == 0 && !hist0_ready) {              // later passes: the previous scatter filled the table
+            hist_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, kin, table, nblocks, shift, bins);
             FP_COUNT(ctx, 1);
         }
-        scan_rows_kernel<<<bins, 256, 0, st>>>(ctx->block_hist, ctx->bin_total, nblocks);
+        scan_rows_kernel<<<bins, 256, 0, st>>>(table, ctx->bin_total, nblocks, other);
+        uint32_t* next = (pass + 1 < passes) ? other : nullptr;
         if (pass == 0)
-            scatter_kernel<true><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, ctx->block_hist, ctx->bin_total, nblocks, shift, bins);
+            scatter_kernel<true><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
         else
-            scatter_kernel<false><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, ctx->block_hist, ctx->bin_total, nblocks, shift, bins);
+            scatter_kernel<false><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
         FP_LAUNCH_OK(ctx);
         FP_COUNT(ctx, 2);
         kin = kout; iin = iout;
         kout = (kout == ctx->key_a) ? ctx->key_b : ctx->key_a;
         iout = (iout == ctx->idx_a) ? ctx->idx_b : ctx->idx_a;
     }
+    ctx->hist0_clean = (passes & 1) == 0;             // the last scan zeroed the table the last pass did not use
     fp_mark(ctx, 2, st);
     const int64_t cap = (int64_t)ctx->num_sms * 16;
     const int64_t want = (np + 255) / 256;

@@ -36,10 +36,16 @@ template <bool WRITE_KEYS>
 __global__ void __launch_bounds__(256)
 sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
           float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
-          uint32_t* __restrict__ keys, const __grid_constant__ sw_params P)
+          uint32_t* __restrict__ keys, uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask,
+          const __grid_constant__ sw_params P)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += stride) {
+    const int lane = threadIdx.x & 31;
+    // warp-uniform trip count: the histogram below is a full-warp collective
+    for (int64_t p0 = (int64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31); p0 < np; p0 += stride) {
+        const int64_t p = p0 + lane;
+        uint32_t key = 0xffffffffu;
+        if (p < np) {
         float v0 = vx[p], v1 = vy[p], v2 = vz[p];
         float xp = fmaf(v0, P.dt, x[p]);
         float yp = fmaf(v1, P.dt, y[p]);
@@ -106,13 +112,23 @@ sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __res
         if (WRITE_KEYS) {
             const int32_t ix = fpd_axis_index(xp, P.x0, P.inv_dx, P.nx);
             const int32_t iy = (P.ny > 1) ? fpd_axis_index(yp, P.y0, P.inv_dy, P.ny) : 0;
-            keys[p] = (uint32_t)(iy * P.nx + ix);
+            key = (uint32_t)(iy * P.nx + ix);
+            keys[p] = key;
+        }
+        }
+        // first radix digit histogram of the sort tile this warp's 32 particles fall in (sort.cu): lanes with the
+        // same digit send one aggregated reduction to tile_hist[digit][tile]; the table is zero on entry
+        if (WRITE_KEYS && tile_hist) {
+            const uint32_t d = (p < np) ? (key & digit_mask) : 0xffffffffu;
+            const uint32_t peers = __match_any_sync(0xffffffffu, d);
+            if (p < np && lane == __ffs(peers) - 1)
+                atomicAdd(&tile_hist[(size_t)d * ntiles + (size_t)(p0 / SORT_TILE)], (uint32_t)__popc(peers));
         }
     }
 }
 
 int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
-                     const uint32_t* pid, uint64_t step, uint32_t* keys_out, cudaStream_t st)
+                     const uint32_t* pid, uint64_t step, uint32_t* keys_out, bool with_hist0, cudaStream_t st)
 {
     if (np == 0) return FP_OK;
     const fp_params& q = ctx->p;
@@ -133,8 +149,18 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
     int64_t want = (np + threads - 1) / threads;
     const int64_t cap = (int64_t)ctx->num_sms * 16;
     const int blocks = (int)(want < cap ? want : cap);
-    if (keys_out) sw_kernel<true><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, keys_out, P);
-    else          sw_kernel<false><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, nullptr, P);
+    if (keys_out) {
+        uint32_t* th = nullptr;
+        if (with_hist0) {
+            th = ctx->block_hist;
+            if (!ctx->hist0_clean) FP_CUDA_OK(ctx, cudaMemsetAsync(th, 0, ctx->block_hist_elems * sizeof(uint32_t), st));
+            ctx->hist0_clean = false;
+        }
+        const uint32_t dmask = (1u << fpi_sort_digit_bits(ctx)) - 1u;
+        sw_kernel<true><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, keys_out, th, fp_div_up(np, SORT_TILE), dmask, P);
+    } else {
+        sw_kernel<false><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
+    }
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
     return FP_OK;
@@ -145,5 +171,5 @@ extern "C" int fp_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, floa
 {
     if (!ctx) return FP_ERR_ARG;
     if (np < 0 || (np > 0 && (!x || !y || !vx || !vy || !vz || !pid))) return fp_fail(ctx, FP_ERR_ARG, "fp_stream_walls: null pointer or np < 0");
-    return fpi_stream_walls(ctx, np, x, y, vx, vy, vz, pid, step, nullptr, (cudaStream_t)stream);
+    return fpi_stream_walls(ctx, np, x, y, vx, vy, vz, pid, step, nullptr, false, (cudaStream_t)stream);
 }
