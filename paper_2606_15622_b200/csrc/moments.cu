@@ -16,9 +16,17 @@
 // cells do not fit its staging buffer (dense or huge cells), or unaligned arrays, run the same code on global pointers.
 #include "tiles.cuh"
 
+#ifndef MOM_THREADS
 #define MOM_THREADS 128
+#endif
 #define MOM_WARPS (MOM_THREADS / 32)
 #define MOM_CHUNK_PER_LANE 64
+#ifndef MOM_CAP
+#define MOM_CAP FPW_CAP            // staged elements per array, warp and stage
+#endif
+#ifndef MOM_G8_MIN
+#define MOM_G8_MIN 48.0            // mean particles per cell from which a cell gets 8 lanes instead of 4
+#endif
 
 // One cell per group of G lanes.  bx/by/bz may point to shared or global memory; particle p is at b?[p].
 // INPLACE: the arrays are the warp's private staging copy, pass 1 overwrites v by v - v_pivot.
@@ -172,30 +180,30 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
     constexpr int NREC = FULL ? 29 : 13;
     constexpr int CPW = 32 / G;                          // cells per warp and chunk
     extern __shared__ __align__(16) unsigned char fpw_smem[];
-    float* stage = reinterpret_cast<float*>(fpw_smem);                                   // [MOM_WARPS][2][3][FPW_CAP]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(fpw_smem + (size_t)MOM_WARPS * 6 * FPW_CAP * sizeof(float));
+    float* stage = reinterpret_cast<float*>(fpw_smem);                                   // [MOM_WARPS][2][3][MOM_CAP]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(fpw_smem + (size_t)MOM_WARPS * 6 * MOM_CAP * sizeof(float));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gl = lane & (G - 1), group = lane / G;
     const int64_t nchunks = ((int64_t)ncell + CPW - 1) / CPW;
     const int64_t nw = (int64_t)gridDim.x * MOM_WARPS;
     int64_t chunk = (int64_t)blockIdx.x * MOM_WARPS + warp;
     if (chunk >= nchunks) return;
-    float* wbuf = stage + (size_t)warp * 6 * FPW_CAP;
+    float* wbuf = stage + (size_t)warp * 6 * MOM_CAP;
     uint64_t* wbar = bars + warp * 2;
     if (lane == 0) { fpt_mbar_init(&wbar[0], 1); fpt_mbar_init(&wbar[1], 1); }
     __syncwarp();
     auto load_cs = [&](int64_t c) { return cell_start[min(c * CPW + lane, (int64_t)ncell)]; };
     auto range_of = [&](int32_t cs) {
-        return fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, aligned != 0);
+        return fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, aligned != 0, MOM_CAP);
     };
     auto issue = [&](const fpw_range& r, int b) {
         const uint32_t bytes = (uint32_t)r.nb * 4u;
         if (r.staged && bytes > 0 && lane == 0) {
-            float* d = wbuf + (size_t)b * 3 * FPW_CAP;
+            float* d = wbuf + (size_t)b * 3 * MOM_CAP;
             fpt_mbar_expect_tx(&wbar[b], 3u * bytes);
             fpt_bulk_g2s(d, vx + r.a0, bytes, &wbar[b]);
-            fpt_bulk_g2s(d + FPW_CAP, vy + r.a0, bytes, &wbar[b]);
-            fpt_bulk_g2s(d + 2 * FPW_CAP, vz + r.a0, bytes, &wbar[b]);
+            fpt_bulk_g2s(d + MOM_CAP, vy + r.a0, bytes, &wbar[b]);
+            fpt_bulk_g2s(d + 2 * MOM_CAP, vz + r.a0, bytes, &wbar[b]);
         }
     };
     int32_t cs_cur = load_cs(chunk);
@@ -221,9 +229,9 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
         const int32_t n = have ? e - s : 0;
         double* rec = mom + (size_t)(have ? cell : 0) * NREC;
         if (r_cur.staged) {
-            float* sx = wbuf + (size_t)b * 3 * FPW_CAP;
-            float* sy = sx + FPW_CAP;
-            float* sz = sy + FPW_CAP;
+            float* sx = wbuf + (size_t)b * 3 * MOM_CAP;
+            float* sy = sx + MOM_CAP;
+            float* sz = sy + MOM_CAP;
             // the (at most 3) particles beyond the last multiple of 4 of the whole array
             for (int32_t p = r_cur.a0 + r_cur.nb + lane; p < r_cur.s1; p += 32) {
                 sx[p - r_cur.a0] = vx[p]; sy[p - r_cur.a0] = vy[p]; sz[p - r_cur.a0] = vz[p];
@@ -247,7 +255,7 @@ static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float
 {
     const int cells_per_block = MOM_WARPS * (32 / G);
     const int aligned = ((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0 ? 1 : 0;
-    const size_t smem = (size_t)MOM_WARPS * 6 * FPW_CAP * sizeof(float) + MOM_WARPS * 2 * sizeof(uint64_t);
+    const size_t smem = (size_t)MOM_WARPS * 6 * MOM_CAP * sizeof(float) + MOM_WARPS * 2 * sizeof(uint64_t);
     static int occ = 0;                           // resident CTAs per SM, one value per instantiation (G)
     if (occ == 0) {
         cudaFuncSetAttribute(moments_warp_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -272,7 +280,7 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     const double ppc = (double)np / (double)ctx->ncell;
     // group width: about 8-16 particles per lane
     if (ppc >= 192.0)      launch_moments<16>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    else if (ppc >= 48.0)  launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else if (ppc >= MOM_G8_MIN)  launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
     else                   launch_moments<4>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);

@@ -81,7 +81,7 @@ struct fpw_range {
     bool staged;           // false: the slice does not fit FPW_CAP or the arrays are not 16-byte aligned
 };
 
-__device__ __forceinline__ fpw_range fpw_range_of(int32_t s0, int32_t s1, int64_t np, bool aligned)
+__device__ __forceinline__ fpw_range fpw_range_of(int32_t s0, int32_t s1, int64_t np, bool aligned, int32_t cap = FPW_CAP)
 {
     fpw_range r;
     r.s0 = s0; r.s1 = s1;
@@ -89,7 +89,7 @@ __device__ __forceinline__ fpw_range fpw_range_of(int32_t s0, int32_t s1, int64_
     const int32_t np4 = (int32_t)(np & ~(int64_t)3);
     const int32_t end4 = min((s1 + 3) & ~3, np4);
     r.nb = max(end4 - r.a0, 0);
-    r.staged = aligned && s1 > s0 && (s1 - r.a0) <= FPW_CAP;
+    r.staged = aligned && s1 > s0 && (s1 - r.a0) <= cap;
     return r;
 }
 
