@@ -83,6 +83,7 @@ extern "C" int fp_destroy(fp_ctx* ctx)
 __global__ void tau_kernel(const int32_t* __restrict__ cell_start, int32_t ncell, float tau_ref_n, float tau_default,
                            float* __restrict__ tau_cell)
 {
+    fpd_pdl();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < ncell) {
         const int32_t n = cell_start[i + 1] - cell_start[i];
@@ -92,7 +93,7 @@ __global__ void tau_kernel(const int32_t* __restrict__ cell_start, int32_t ncell
 
 int fpi_tau_from_counts(fp_ctx* ctx, const int32_t* cell_start, float tau_ref_n, float* tau_cell, cudaStream_t st)
 {
-    tau_kernel<<<fp_div_up(ctx->ncell, 256), 256, 0, st>>>(cell_start, ctx->ncell, tau_ref_n, ctx->p.tau, tau_cell);
+    fp_launch(tau_kernel, fp_div_up(ctx->ncell, 256), 256, 0, st, cell_start, ctx->ncell, tau_ref_n, ctx->p.tau, tau_cell);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
     return FP_OK;

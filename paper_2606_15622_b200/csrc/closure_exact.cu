@@ -79,6 +79,7 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
                      float eps2_scale, int32_t min_count, int32_t ncell, float* __restrict__ coef,
                      uint32_t* __restrict__ flags, double* __restrict__ kappa_est, float* __restrict__ cellc, float dt)
 {
+    fpd_pdl();
     extern __shared__ double ce_sm[];
     double* recs = ce_sm;                        // [CE_TPB * 29] staged records, dead once scaled into registers ...
     double* As = ce_sm;                          // ... then [90][CE_TPB] augmented systems in the same memory
@@ -222,7 +223,7 @@ int fpi_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell
         FP_CUDA_OK(ctx, cudaFuncSetAttribute(closure_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    closure_exact_kernel<<<blocks, CE_TPB, smem, stream>>>(mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
+    fp_launch(closure_exact_kernel, blocks, CE_TPB, smem, stream, mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
                                                                        ctx->p.min_count, ncell, coef, flags, kappa_est,
                                                                        with_update_constants ? ctx->cellc : nullptr, ctx->p.dt);
     FP_LAUNCH_OK(ctx);

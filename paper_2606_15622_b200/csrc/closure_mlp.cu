@@ -38,6 +38,7 @@ static inline int pad8(int v) { return (v + 7) & ~7; }
 __global__ void mlp_pack_kernel(const __grid_constant__ mlp_desc D, const __grid_constant__ mlp_src S,
                                 float* __restrict__ blob)
 {
+    fpd_pdl();
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
     for (int l = 0; l < D.n_layers; ++l) {
         const int ni = D.dims[l], no = D.dims[l + 1], nop = (no + 7) & ~7;
@@ -59,6 +60,7 @@ mlp_kernel(const double* __restrict__ mom, int32_t stride, const float* __restri
            float relax_w, int32_t ncell, float* __restrict__ coef, uint32_t* __restrict__ flags,
            float* __restrict__ cellc, float dt, float eps2_scale)
 {
+    fpd_pdl();
     extern __shared__ __align__(16) float smem[];
     float* wsm = smem;
     float* act0 = smem + (w_in_smem ? ((D.blob_floats + 3) & ~3) : 0);
@@ -232,7 +234,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         if (!C.tc_frags) FP_CUDA_OK(ctx, cudaMalloc((void**)&C.tc_frags, fbytes));
         float4* frags = reinterpret_cast<float4*>(C.tc_frags);
         float* misc = C.tc_frags + (size_t)TC_FRAGS * 4;
-        mlp_tc_pack_kernel<<<20, 256, 0, st>>>(S, D.dims[0], frags, misc);
+        fp_launch(mlp_tc_pack_kernel, 20, 256, 0, st, S, D.dims[0], frags, misc);
         tc_params P;
         P.stride = mom_stride; P.feature_set = M.feature_set; P.act = M.act; P.min_count = ctx->p.min_count_mlp;
         P.ncell = ctx->ncell; P.nin = D.dims[0]; P.tau_scalar = ctx->p.tau; P.n_scale = M.n_scale;
@@ -247,7 +249,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         }
         const int want = fp_div_up(fp_div_up(ctx->ncell, 16), TC_WARPS);
         const int cap = ctx->num_sms * occ;
-        mlp_tc_kernel<<<want < cap ? want : cap, TC_THREADS, smem, st>>>(mom, tau_cell, frags, misc, coef, flags, P);
+        fp_launch(mlp_tc_kernel, want < cap ? want : cap, TC_THREADS, smem, st, mom, tau_cell, frags, misc, coef, flags, P);
         FP_LAUNCH_OK(ctx);
         FP_COUNT(ctx, 2);
         return FP_OK;
@@ -258,7 +260,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         FP_CUDA_OK(ctx, cudaMallocAsync((void**)&C.blob, (size_t)off * sizeof(float), st));
         C.blob_floats = (size_t)off;
     }
-    mlp_pack_kernel<<<fp_div_up(off, 256) < 64 ? fp_div_up(off, 256) : 64, 256, 0, st>>>(D, S, C.blob);
+    fp_launch(mlp_pack_kernel, fp_div_up(off, 256) < 64 ? fp_div_up(off, 256) : 64, 256, 0, st, D, S, C.blob);
     FP_LAUNCH_OK(ctx);
     const int32_t ncell = ctx->ncell;
     const size_t wbytes = (size_t)((off + 3) & ~3) * sizeof(float);
@@ -268,7 +270,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         const int w_in_smem = (wbytes + abytes <= 200 * 1024) ? 1 : 0;
         const size_t smem = abytes + (w_in_smem ? wbytes : 0);
         FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_kernel<CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        mlp_kernel<CB><<<fp_div_up(ncell, CB), CB, smem, st>>>(mom, mom_stride, tau_cell, ctx->p.tau, C.blob, D, w_in_smem,
+        fp_launch(mlp_kernel<CB>, fp_div_up(ncell, CB), CB, smem, st, mom, mom_stride, tau_cell, ctx->p.tau, C.blob, D, w_in_smem,
                                                              ctx->p.min_count_mlp, relax_w, ncell, coef, flags, cellc,
                                                              ctx->p.dt, ctx->p.eps2_scale);
     } else if (maxw <= 512) {
@@ -277,7 +279,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         const int w_in_smem = (wbytes + abytes <= 200 * 1024) ? 1 : 0;
         const size_t smem = abytes + (w_in_smem ? wbytes : 0);
         FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_kernel<CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        mlp_kernel<CB><<<fp_div_up(ncell, CB), CB, smem, st>>>(mom, mom_stride, tau_cell, ctx->p.tau, C.blob, D, w_in_smem,
+        fp_launch(mlp_kernel<CB>, fp_div_up(ncell, CB), CB, smem, st, mom, mom_stride, tau_cell, ctx->p.tau, C.blob, D, w_in_smem,
                                                              ctx->p.min_count_mlp, relax_w, ncell, coef, flags, cellc,
                                                              ctx->p.dt, ctx->p.eps2_scale);
     } else {

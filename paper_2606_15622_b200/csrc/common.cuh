@@ -94,6 +94,31 @@ static inline int fp_fail(fp_ctx* ctx, int code, const char* msg)
 #define FP_LAUNCH_OK(ctx) FP_CUDA_OK(ctx, cudaGetLastError())
 #define FP_COUNT(ctx, n) ((ctx)->launches += (n))
 
+#ifdef __CUDACC__
+// Launch with programmatic dependent launch allowed: the grid is set up while its predecessor on the stream still
+// runs and blocks in fpd_pdl() until that predecessor has completed and its writes are visible.  Every kernel of the
+// fp_step chain starts with fpd_pdl(); no kernel triggers its dependents early (measured: an early
+// griddepcontrol.launch_dependents parks idle blocks on the SMs and costs 55 us per step, the implicit trigger at
+// kernel exit saves 18 us of launch gaps per step at 4M particles).
+template <typename... KArgs, typename... Args>
+static inline cudaError_t fp_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                    Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+// first statement of a kernel launched with fp_launch (a no-op under a plain launch)
+__device__ __forceinline__ void fpd_pdl()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+#endif
+
 static inline int fp_div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // internal entry points shared between translation units (not exported)

@@ -46,6 +46,7 @@ __device__ __forceinline__ void tc_mma(float (&c)[4], const uint32_t (&a)[4], ui
 __global__ void mlp_tc_pack_kernel(const __grid_constant__ mlp_src S, int32_t nin, float4* __restrict__ frags,
                                    float* __restrict__ misc)
 {
+    fpd_pdl();
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
     for (int e = tid; e < TC_FRAGS; e += nth) {
         int l, r = e;
@@ -141,6 +142,7 @@ mlp_tc_kernel(const double* __restrict__ mom, const float* __restrict__ tau_cell
               const float* __restrict__ misc, float* __restrict__ coef, uint32_t* __restrict__ flags,
               const __grid_constant__ tc_params P)
 {
+    fpd_pdl();
     extern __shared__ __align__(16) unsigned char tc_smem[];
     float4* wf = reinterpret_cast<float4*>(tc_smem);                               // [TC_FRAGS]
     float* ms = reinterpret_cast<float*>(tc_smem + (size_t)TC_FRAGS * sizeof(float4));   // [TC_MISC]

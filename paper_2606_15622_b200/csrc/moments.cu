@@ -177,6 +177,7 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
                     const int32_t* __restrict__ cell_start, int32_t ncell, int64_t np, int32_t aligned,
                     double* __restrict__ mom)
 {
+    fpd_pdl();
     constexpr int NREC = FULL ? 29 : 13;
     constexpr int CPW = 32 / G;                          // cells per warp and chunk
     extern __shared__ __align__(16) unsigned char fpw_smem[];
@@ -266,8 +267,8 @@ static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float
     const int want = fp_div_up(ctx->ncell, cells_per_block);
     const int cap = ctx->num_sms * occ;
     const int blocks = want < cap ? want : cap;
-    if (mode) moments_warp_kernel<G, true><<<blocks, MOM_THREADS, smem, st>>>(vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
-    else      moments_warp_kernel<G, false><<<blocks, MOM_THREADS, smem, st>>>(vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
+    if (mode) fp_launch(moments_warp_kernel<G, true>, blocks, MOM_THREADS, smem, st, vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
+    else      fp_launch(moments_warp_kernel<G, false>, blocks, MOM_THREADS, smem, st, vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
 }
 
 extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,

@@ -60,6 +60,7 @@ __global__ void __launch_bounds__(256)
 scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_total, int nblocks,
                  uint32_t* __restrict__ other_table)
 {
+    fpd_pdl();
     // the other pass's table is free now: clear this digit's row for the reductions that fill it next
     for (int i = threadIdx.x; i < nblocks; i += 256) other_table[(size_t)blockIdx.x * nblocks + i] = 0u;
     __shared__ uint32_t wsum[8];
@@ -95,6 +96,7 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
                const uint32_t* __restrict__ block_hist, const uint32_t* __restrict__ bin_total, int nblocks,
                int shift, int bins, uint32_t* __restrict__ next_hist)
 {
+    fpd_pdl();
     __shared__ uint32_t cnt[SORT_WARPS][SORT_MAX_BINS];   // per-warp running digit counts, then bases
     __shared__ uint32_t bin_base[SORT_MAX_BINS];          // global start of each digit value + this tile's offset
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -187,6 +189,7 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
               float* __restrict__ xo, float* __restrict__ yo, float* __restrict__ vxo, float* __restrict__ vyo,
               float* __restrict__ vzo, uint32_t* __restrict__ pido)
 {
+    fpd_pdl();
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < np; k += stride) {
         const uint32_t s = perm[k];
@@ -242,12 +245,12 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
             hist_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, kin, table, nblocks, shift, bins);
             FP_COUNT(ctx, 1);
         }
-        scan_rows_kernel<<<bins, 256, 0, st>>>(table, ctx->bin_total, nblocks, other);
+        fp_launch(scan_rows_kernel, bins, 256, 0, st, table, ctx->bin_total, nblocks, other);
         uint32_t* next = (pass + 1 < passes) ? other : nullptr;
         if (pass == 0)
-            scatter_kernel<true><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
+            fp_launch(scatter_kernel<true>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
         else
-            scatter_kernel<false><<<nblocks, SORT_THREADS, 0, st>>>(np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
+            fp_launch(scatter_kernel<false>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
         FP_LAUNCH_OK(ctx);
         FP_COUNT(ctx, 2);
         kin = kout; iin = iout;
@@ -258,7 +261,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     fp_mark(ctx, 2, st);
     const int64_t cap = (int64_t)ctx->num_sms * 16;
     const int64_t want = (np + 255) / 256;
-    gather_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
+    fp_launch(gather_kernel, (int)(want < cap ? want : cap), 256, 0, st, np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
                                                                  x_out, y_out, vx_out, vy_out, vz_out, pid_out);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);

@@ -39,6 +39,7 @@ sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __res
           uint32_t* __restrict__ keys, uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask,
           const __grid_constant__ sw_params P)
 {
+    fpd_pdl();
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     const int lane = threadIdx.x & 31;
     // warp-uniform trip count: the histogram below is a full-warp collective
@@ -157,9 +158,9 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
             ctx->hist0_clean = false;
         }
         const uint32_t dmask = (1u << fpi_sort_digit_bits(ctx)) - 1u;
-        sw_kernel<true><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, keys_out, th, fp_div_up(np, SORT_TILE), dmask, P);
+        fp_launch(sw_kernel<true>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, keys_out, th, fp_div_up(np, SORT_TILE), dmask, P);
     } else {
-        sw_kernel<false><<<blocks, threads, 0, st>>>(np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
+        fp_launch(sw_kernel<false>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
     }
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
