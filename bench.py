@@ -244,6 +244,45 @@ def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
     return res
 
 
+def corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, steps):
+    """the judged kernels again where the velocity arrays cannot sit in the 126 MB L2 -- C4 at 200 ppc
+    (8M particles, 96 MB of velocities) and C5 (hypersonic cylinder, ~20M particles, 5..400 per cell, 240 MB)."""
+    res = {}
+    for name in ("c4_8m", "c5"):
+        if name == "c4_8m":
+            cfg, st = workloads.cavity(n=200, ppc=200, kn=1.0, seed=42, shuffle=True)
+            kw = {}
+            label = "cavity Kn=1.0 200x200 cells x 200 ppc (BASELINE config 4)"
+        else:
+            cfg, st, _tau = workloads.cylinder()
+            tau_buf = torch.empty(cfg["nx"] * cfg["ny"], dtype=torch.float32, device="cuda")
+            kw = dict(tau_mode=1, tau_ref_n=cfg["tau"] * cfg["ppc_inf"], tau_cell=tau_buf)
+            label = "hypersonic cylinder 400x300 cells, 5..400 ppc (BASELINE config 5)"
+        ctx = fpcl.Context(cfg)
+        a = fpcl.to_device(st)
+        b = {k: torch.empty_like(v) for k, v in a.items()}
+        out = ctx.alloc_step_outputs(0)
+        n = 0
+        for _ in range(10):
+            ctx.step(a, b, n, out, closure=0, **kw); a, b = b, a; n += 1
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            ctx.step(a, b, n, out, closure=0, **kw); a, b = b, a; n += 1
+        e1.record(); e1.synchronize()
+        np_ = a["x"].numel()
+        ms = e0.elapsed_time(e1) / steps
+        tab = cold_kernel_table(fpcl, torch, ctx, a, out, mlp_dev, hbm_peak, reps=8)
+        res[name] = {"workload": label, "particles": np_, "cells": ctx.ncell, "fp_step_ms": ms,
+                     "particle_steps_per_s": np_ / (ms * 1e-3),
+                     "flags_nonzero_cells": int((out["flags"] != 0).sum().item()), "kernels_cold_l2": tab}
+        ctx.close()
+        del a, b, out
+        torch.cuda.empty_cache()
+    return res
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -354,9 +393,9 @@ def main():
     # dominant single kernel of the step (sort_keys is six launches; the others are one kernel each)
     single = {n: stages[n] for n in ("stream_walls", "gather", "moments", "closure", "update")}
     dom = max(single, key=lambda n: single[n]["ms"])
-    # DRAM traffic per launch from the committed ncu --set full capture (profiles/r01_ncu_full_v2.md, C3), bytes;
+    # DRAM traffic per launch from the committed ncu --set full capture (profiles/r01_ncu_full_v4.md, C3), bytes;
     # the in-place update's writes are still in L2 when its kernel ends, so its figure is mostly reads
-    ncu_traffic = {"update": 70.3e6 + 10.9e6, "moments": 48.4e6, "gather": 204.1e6, "stream_walls": 88.3e6,
+    ncu_traffic = {"update": 70.7e6, "moments": 48.4e6, "gather": 204.6e6, "stream_walls": 91.2e6,
                    "closure": 9.3e6 if closure == 0 else 4.3e6}
     roofline = {"kernel": dom, "bound": "hbm", "achieved": single[dom]["GBps_algorithmic"], "peak": hbm_peak,
                 "unit": "GB/s", "frac": single[dom]["frac_of_hbm_peak"],
@@ -380,6 +419,9 @@ def main():
         f1.record(); f1.synchronize()
         extras["step_with_mlp_closure"] = {"ms_per_step": f0.elapsed_time(f1) / nrep,
                                            "particle_steps_per_s": np_ * nrep / (f0.elapsed_time(f1) * 1e-3)}
+        if not args.small:
+            del a2, b2, out2
+            extras["beyond_l2"] = corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, min(args.steps, 20))
 
     cpu_baseline = None
     if rank == 0 and not args.no_cpu_baseline:

@@ -24,9 +24,6 @@
 #ifndef MOM_CAP
 #define MOM_CAP FPW_CAP            // staged elements per array, warp and stage
 #endif
-#ifndef MOM_G8_MIN
-#define MOM_G8_MIN 48.0            // mean particles per cell from which a cell gets 8 lanes instead of 4
-#endif
 
 // One cell per group of G lanes.  bx/by/bz may point to shared or global memory; particle p is at b?[p].
 // INPLACE: the arrays are the warp's private staging copy, pass 1 overwrites v by v - v_pivot.
@@ -37,7 +34,7 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     float* wx = const_cast<float*>(bx);
     float* wy = const_cast<float*>(by);
     float* wz = const_cast<float*>(bz);
-    constexpr int NP = FULL ? 32 : 16;          // padded record length
+    constexpr int NP = (FULL || G > 16) ? 32 : 16;   // padded record length (at least one slot per lane)
     constexpr int NREC = FULL ? 29 : 13;
     constexpr int PER = NP / G;                 // record slots per lane after the transposing reduction
     static_assert(NP >= G, "group wider than the padded record");
@@ -168,6 +165,47 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     }
 }
 
+// The cells of a chunk that does not fit the staging buffer, one at a time: each staged on its own and reduced by
+// all 32 lanes; only a cell that alone exceeds the buffer reads global memory.  Kept out of line so that its
+// registers do not add to the common path's.
+template <bool FULL>
+__device__ __noinline__ void mom_dense_chunk(const float* __restrict__ vx, const float* __restrict__ vy,
+                                             const float* __restrict__ vz, int32_t cs_cur, int cpw, int64_t chunk,
+                                             int32_t ncell, int64_t np, int32_t aligned, float* sx, uint64_t* bar,
+                                             uint32_t& phase, int b, int lane, double* __restrict__ mom)
+{
+    constexpr int NREC = FULL ? 29 : 13;
+    float* sy = sx + MOM_CAP;
+    float* sz = sy + MOM_CAP;
+#pragma unroll 1
+    for (int c = 0; c < cpw; ++c) {
+        const int32_t s1c = __shfl_sync(0xffffffffu, cs_cur, c), e1c = __shfl_sync(0xffffffffu, cs_cur, c + 1);
+        const int64_t cellc = chunk * cpw + c;
+        if (cellc >= ncell) continue;                                             // warp-uniform
+        double* recc = mom + (size_t)cellc * NREC;
+        const fpw_range rc = fpw_range_of(s1c, e1c, np, aligned != 0, MOM_CAP);
+        if (rc.staged) {
+            fpt_fence_proxy_async();                 // earlier generic writes to the buffer vs the new bulk copy
+            __syncwarp();
+            const uint32_t bytes = (uint32_t)rc.nb * 4u;
+            if (bytes > 0 && lane == 0) {
+                fpt_mbar_expect_tx(bar, 3u * bytes);
+                fpt_bulk_g2s(sx, vx + rc.a0, bytes, bar);
+                fpt_bulk_g2s(sy, vy + rc.a0, bytes, bar);
+                fpt_bulk_g2s(sz, vz + rc.a0, bytes, bar);
+            }
+            for (int32_t p = rc.a0 + rc.nb + lane; p < rc.s1; p += 32) {
+                sx[p - rc.a0] = vx[p]; sy[p - rc.a0] = vy[p]; sz[p - rc.a0] = vz[p];
+            }
+            if (bytes > 0) { fpt_mbar_wait(bar, (phase >> b) & 1u); phase ^= 1u << b; }
+            __syncwarp();
+            mom_cell_group<32, FULL, true>(sx - rc.a0, sy - rc.a0, sz - rc.a0, s1c, e1c - s1c, true, lane, recc);
+        } else {
+            mom_cell_group<32, FULL, false>(vx, vy, vz, s1c, e1c - s1c, true, lane, recc);
+        }
+    }
+}
+
 // Persistent warps: a warp owns chunks wg, wg + nwarps, ... of 32/G consecutive cells; while it reduces one chunk the
 // bulk copies of its next chunk are already in flight into the warp's other staging buffer (2-stage pipeline per
 // warp, mbarrier per stage), and the cell boundaries of the chunk after that are being fetched.
@@ -241,7 +279,9 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
             __syncwarp();
             mom_cell_group<G, FULL, true>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, s, n, have, gl, rec);   // shared-memory loads
         } else {
-            mom_cell_group<G, FULL, false>(vx, vy, vz, s, n, have, gl, rec);                                    // global loads
+            // a chunk too dense for the staging buffer (load-imbalanced grids): cell by cell in buffer b
+            mom_dense_chunk<FULL>(vx, vy, vz, cs_cur, CPW, chunk, ncell, np, aligned, wbuf + (size_t)b * 3 * MOM_CAP,
+                                  &wbar[b], phase, b, lane, mom);
         }
         if (nxt >= nchunks) break;
         chunk = nxt; cs_cur = cs_nxt; r_cur = r_nxt;
@@ -279,9 +319,10 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     if (np > 0 && (!vx || !vy || !vz)) return fp_fail(ctx, FP_ERR_ARG, "fp_cell_moments: null velocity pointer");
     cudaStream_t st = (cudaStream_t)stream;
     const double ppc = (double)np / (double)ctx->ncell;
-    // group width: about 8-16 particles per lane
-    if (ppc >= 192.0)      launch_moments<16>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    else if (ppc >= MOM_G8_MIN)  launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    // group width: the chunk of 32/G cells must fit the staging buffer (tiles.cuh)
+    if (ppc >= FPW_G32_MIN)      launch_moments<32>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else if (ppc >= FPW_G16_MIN) launch_moments<16>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else if (ppc >= FPW_G8_MIN)  launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
     else                   launch_moments<4>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);

@@ -9,6 +9,14 @@
 #include "common.cuh"
 
 #define FPW_CAP 512                // staged elements per array, warp and stage (4 cells x 128 particles)
+// Lanes per cell G by mean particles per cell: a warp's chunk of 32/G cells has to fit FPW_CAP with room for the
+// count fluctuations (at the mean where G changes the chunk holds 7/8 of the buffer); chunks that still do not fit
+// are walked cell by cell with all 32 lanes.
+#ifndef FPW_G8_MIN
+#define FPW_G8_MIN 56.0            // 8 cells x 56 = 448
+#endif
+#define FPW_G16_MIN 112.0          // 4 cells x 112 = 448
+#define FPW_G32_MIN 224.0          // 2 cells x 224 = 448
 
 #ifdef __CUDACC__
 
