@@ -2,7 +2,9 @@
 // DESIGN.md R1).  Integer work: results are bit-exact and unique (equal keys keep input order).
 //
 // Least-significant-digit radix sort on (key, index) pairs, digit width <= 9 bits so that a 2^18-cell grid sorts
-// in two passes.  Each pass = per-tile digit histogram -> per-digit scan over tiles -> stable scatter.  Stability
+// in two passes.  Each pass = per-tile digit histogram -> per-digit scan over tiles -> stable scatter; the histogram
+// of a pass is produced by whoever writes that pass's input (key_kernel / the stream kernel for the first pass, the
+// previous scatter for the later ones), hist_kernel only serves callers that bring their own keys.  Stability
 // inside a tile comes from warp-striped item order plus __match_any_sync ranking (no atomics decide an order).
 // The payload (x, y, vx, vy, vz, pid) is gathered once at the end through the final permutation.
 #include "common.cuh"
@@ -83,61 +85,34 @@ scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_t
     if (tid == 0) bin_total[blockIdx.x] = total;
 }
 
-// stable scatter of one tile.  Warp w owns items [w*256, (w+1)*256) of the tile in warp-striped order
-// (round i, lane l -> w*256 + i*32 + l), so (tile, warp, round, lane) order is input order.
-#ifndef SORT_SCATTER_MINB
-#define SORT_SCATTER_MINB 4                               // 64 registers: four tiles per SM hide the latency phases
-#endif
 __device__ __forceinline__ int dbits_of(int bins) { return 31 - __clz(bins); }
-template <bool FIRST_PASS>
-__global__ void __launch_bounds__(SORT_THREADS, SORT_SCATTER_MINB)
-scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
-               uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out,
-               const uint32_t* __restrict__ block_hist, const uint32_t* __restrict__ bin_total, int nblocks,
-               int shift, int bins, uint32_t* __restrict__ next_hist)
+
+// The items of one tile: load, rank, scatter.  FULLT: every item of the tile exists (no bounds checks).
+template <bool FIRST_PASS, bool FULLT>
+__device__ __forceinline__ void scatter_items(int64_t np, const uint32_t* __restrict__ keys_in,
+                                              const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ keys_out,
+                                              uint32_t* __restrict__ idx_out, int nblocks, int shift, int bins,
+                                              uint32_t* __restrict__ next_hist, uint32_t (*cnt)[SORT_MAX_BINS],
+                                              const uint32_t* bin_base)
 {
-    fpd_pdl();
-    __shared__ uint32_t cnt[SORT_WARPS][SORT_MAX_BINS];   // per-warp running digit counts, then bases
-    __shared__ uint32_t bin_base[SORT_MAX_BINS];          // global start of each digit value + this tile's offset
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t mask = (uint32_t)bins - 1u;
-    for (int b = threadIdx.x; b < bins * SORT_WARPS; b += SORT_THREADS) (&cnt[0][0])[(b / bins) * SORT_MAX_BINS + (b % bins)] = 0;
-    // exclusive scan of the digit totals (bins <= 512 = 8 warps x 32 lanes x 2 consecutive bins): every thread fetches
-    // its two totals and its two tile offsets at once (one global latency), warps scan, warp totals go through smem
-    {
-        __shared__ uint32_t wtot[SORT_WARPS];
-        const int b0 = 2 * (int)threadIdx.x, b1 = b0 + 1;
-        const uint32_t v0 = (b0 < bins) ? bin_total[b0] : 0u, v1 = (b1 < bins) ? bin_total[b1] : 0u;
-        const uint32_t h0 = (b0 < bins) ? block_hist[(size_t)b0 * nblocks + blockIdx.x] : 0u;
-        const uint32_t h1 = (b1 < bins) ? block_hist[(size_t)b1 * nblocks + blockIdx.x] : 0u;
-        uint32_t incl = v0 + v1;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
-        if (lane == 31) wtot[warp] = incl;
-        __syncthreads();
-        uint32_t wb = 0;
-#pragma unroll
-        for (int w = 0; w < SORT_WARPS; ++w) if (w < warp) wb += wtot[w];
-        const uint32_t e = wb + incl - (v0 + v1);
-        if (b0 < bins) bin_base[b0] = e + h0;
-        if (b1 < bins) bin_base[b1] = e + v0 + h1;
-    }
-    __syncthreads();
-    const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS);
+    const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS) + lane;   // this lane's first item
+    const uint32_t* kp = keys_in + wbase;
+    const uint32_t* ip = FIRST_PASS ? nullptr : idx_in + wbase;
     uint32_t key[SORT_ITEMS], idx[SORT_ITEMS], rank[SORT_ITEMS];
     bool valid[SORT_ITEMS];
 #pragma unroll
     for (int i = 0; i < SORT_ITEMS; ++i) {
-        const int64_t p = wbase + i * 32 + lane;
-        valid[i] = p < np;
-        key[i] = valid[i] ? keys_in[p] : 0xffffffffu;
-        idx[i] = FIRST_PASS ? (uint32_t)p : (valid[i] ? idx_in[p] : 0u);
+        valid[i] = FULLT ? true : (wbase + i * 32 < np);
+        key[i] = valid[i] ? kp[i * 32] : 0xffffffffu;
+        idx[i] = FIRST_PASS ? (uint32_t)wbase + (uint32_t)(i * 32) : (valid[i] ? ip[i * 32] : 0u);
     }
     // rank inside the warp's sub-tile, round by round (stable)
 #pragma unroll
     for (int i = 0; i < SORT_ITEMS; ++i) {
         const uint32_t d = (key[i] >> shift) & mask;
-        const uint32_t act = __ballot_sync(0xffffffffu, valid[i]);
+        const uint32_t act = FULLT ? 0xffffffffu : __ballot_sync(0xffffffffu, valid[i]);
         uint32_t r = 0;
         if (valid[i]) {
             const uint32_t peers = __match_any_sync(act, d);   // (a ballot-per-bit search measured slower: 111 vs 99 us)
@@ -177,6 +152,54 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
                 atomicAdd(&next_hist[(size_t)(code >> 20) * nblocks + (code & 0xfffffu)], (uint32_t)__popc(peers));
         }
     }
+}
+
+// stable scatter of one tile.  Warp w owns items [w*256, (w+1)*256) of the tile in warp-striped order
+// (round i, lane l -> w*256 + i*32 + l), so (tile, warp, round, lane) order is input order.
+#ifndef SORT_SCATTER_MINB
+#define SORT_SCATTER_MINB 4                               // 64 registers: four tiles per SM hide the latency phases
+#endif
+template <bool FIRST_PASS>
+__global__ void __launch_bounds__(SORT_THREADS, SORT_SCATTER_MINB)
+scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
+               uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out,
+               const uint32_t* __restrict__ block_hist, const uint32_t* __restrict__ bin_total, int nblocks,
+               int shift, int bins, uint32_t* __restrict__ next_hist)
+{
+    fpd_pdl();
+    __shared__ uint32_t cnt[SORT_WARPS][SORT_MAX_BINS];   // per-warp running digit counts, then bases
+    __shared__ uint32_t bin_base[SORT_MAX_BINS];          // global start of each digit value + this tile's offset
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t mask = (uint32_t)bins - 1u;
+    for (int b = threadIdx.x; b < bins; b += SORT_THREADS) {          // bins is a power of two <= SORT_MAX_BINS
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) cnt[w][b] = 0;
+    }
+    // exclusive scan of the digit totals (bins <= 512 = 8 warps x 32 lanes x 2 consecutive bins): every thread fetches
+    // its two totals and its two tile offsets at once (one global latency), warps scan, warp totals go through smem
+    {
+        __shared__ uint32_t wtot[SORT_WARPS];
+        const int b0 = 2 * (int)threadIdx.x, b1 = b0 + 1;
+        const uint32_t v0 = (b0 < bins) ? bin_total[b0] : 0u, v1 = (b1 < bins) ? bin_total[b1] : 0u;
+        const uint32_t h0 = (b0 < bins) ? block_hist[(size_t)b0 * nblocks + blockIdx.x] : 0u;
+        const uint32_t h1 = (b1 < bins) ? block_hist[(size_t)b1 * nblocks + blockIdx.x] : 0u;
+        uint32_t incl = v0 + v1;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
+        if (lane == 31) wtot[warp] = incl;
+        __syncthreads();
+        uint32_t wb = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) if (w < warp) wb += wtot[w];
+        const uint32_t e = wb + incl - (v0 + v1);
+        if (b0 < bins) bin_base[b0] = e + h0;
+        if (b1 < bins) bin_base[b1] = e + v0 + h1;
+    }
+    __syncthreads();
+    if ((int64_t)(blockIdx.x + 1) * SORT_TILE <= np)       // block-uniform: all but the last tile are full
+        scatter_items<FIRST_PASS, true>(np, keys_in, idx_in, keys_out, idx_out, nblocks, shift, bins, next_hist, cnt, bin_base);
+    else
+        scatter_items<FIRST_PASS, false>(np, keys_in, idx_in, keys_out, idx_out, nblocks, shift, bins, next_hist, cnt, bin_base);
 }
 
 // payload permute fused with cell_start from the sorted keys: cell_start[k] = first position whose key >= k,
