@@ -1,8 +1,8 @@
 // stream_walls.cu -- a0 + a1: streaming (Eq. 16 :187) and diffuse isothermal walls (:214, :380, :674;
 // DESIGN.md R7), fused with the cell-key computation of a2 (R1) when called from fp_step.
 //
-// One thread per particle, SoA fp32, fully coalesced: 24 B read (x, y, vx, vy, vz, pid is read only by particles
-// that hit a wall), 8 B written (x, y) + 4 B key; wall hits add 12 B of velocity writes.  HBM-bound.
+// One thread per particle, SoA fp32, fully coalesced: 16 B read (x, y, vx, vy; pid is read only by particles that
+// hit a wall, vz never), 8 B written (x, y) + 4 B key; wall hits add 12 B of velocity writes.
 // Positions follow a fixed fp32 operation sequence (they decide the integer cell index); re-emitted velocities
 // are drawn with fp32 logf / sincospif from the Philox uniforms (tolerance 1e-6 relative).
 #include "common.cuh"
@@ -32,24 +32,16 @@ __device__ __forceinline__ void sw_wall_draw(const sw_params& P, uint32_t pid, u
     t2 = r * s;
 }
 
+// One particle: stream, walls, body, key.  pid is read only by particles that hit something.
+struct sw_moved { float x, y, v0, v1, v2; uint32_t key; bool redrawn; };
+
 template <bool WRITE_KEYS>
-__global__ void __launch_bounds__(256)
-sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
-          float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
-          uint32_t* __restrict__ keys, uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask,
-          const __grid_constant__ sw_params P)
+__device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float yin, float v0, float v1,
+                                            const uint32_t* __restrict__ pid, int64_t p)
 {
-    fpd_pdl();
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int lane = threadIdx.x & 31;
-    // warp-uniform trip count: the histogram below is a full-warp collective
-    for (int64_t p0 = (int64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31); p0 < np; p0 += stride) {
-        const int64_t p = p0 + lane;
-        uint32_t key = 0xffffffffu;
-        if (p < np) {
-        float v0 = vx[p], v1 = vy[p], v2 = vz[p];
-        float xp = fmaf(v0, P.dt, x[p]);
-        float yp = fmaf(v1, P.dt, y[p]);
+        float v2 = 0.0f;                           // vz is only ever replaced, never read
+        float xp = fmaf(v0, P.dt, xin);
+        float yp = fmaf(v1, P.dt, yin);
         bool redrawn = false;
         // x pair
         {
@@ -108,23 +100,51 @@ sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __res
                 v0 = vn * nxn - t1 * nyn; v1 = vn * nyn + t1 * nxn; v2 = t2; redrawn = true;
             }
         }
-        x[p] = xp; y[p] = yp;
-        if (redrawn) { vx[p] = v0; vy[p] = v1; vz[p] = v2; }
+        sw_moved m;
+        m.x = xp; m.y = yp; m.v0 = v0; m.v1 = v1; m.v2 = v2; m.redrawn = redrawn; m.key = 0u;
         if (WRITE_KEYS) {
             const int32_t ix = fpd_axis_index(xp, P.x0, P.inv_dx, P.nx);
             const int32_t iy = (P.ny > 1) ? fpd_axis_index(yp, P.y0, P.inv_dy, P.ny) : 0;
-            key = (uint32_t)(iy * P.nx + ix);
-            keys[p] = key;
+            m.key = (uint32_t)(iy * P.nx + ix);
         }
+        return m;
+}
+
+// first radix digit histogram of the sort tile a warp's particles fall in (sort.cu): lanes with the same digit send
+// one aggregated reduction to tile_hist[digit][tile]; the table is zero on entry.  Full-warp collective.
+__device__ __forceinline__ void sw_hist(uint32_t* __restrict__ tile_hist, int ntiles, int64_t tile, bool valid,
+                                        uint32_t key, uint32_t digit_mask, int lane)
+{
+    const uint32_t d = valid ? (key & digit_mask) : 0xffffffffu;
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    if (valid && lane == __ffs(peers) - 1)
+        atomicAdd(&tile_hist[(size_t)d * ntiles + (size_t)tile], (uint32_t)__popc(peers));
+}
+
+// One particle per thread, grid-stride.  (Four particles per thread with 128-bit accesses was measured slower:
+// 37 vs 33 us at 4M particles.)
+template <bool WRITE_KEYS>
+__global__ void __launch_bounds__(256)
+sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
+          float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
+          uint32_t* __restrict__ keys, uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask,
+          const __grid_constant__ sw_params P)
+{
+    fpd_pdl();
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int lane = threadIdx.x & 31;
+    // warp-uniform trip count: the histogram is a full-warp collective; a warp's 32 particles lie in one sort tile
+    for (int64_t p0 = (int64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31); p0 < np; p0 += stride) {
+        const int64_t p = p0 + lane;
+        const bool valid = p < np;
+        uint32_t key = 0u;
+        if (valid) {
+            const sw_moved m = sw_move<WRITE_KEYS>(P, x[p], y[p], vx[p], vy[p], pid, p);
+            x[p] = m.x; y[p] = m.y; key = m.key;
+            if (m.redrawn) { vx[p] = m.v0; vy[p] = m.v1; vz[p] = m.v2; }
+            if (WRITE_KEYS) keys[p] = key;
         }
-        // first radix digit histogram of the sort tile this warp's 32 particles fall in (sort.cu): lanes with the
-        // same digit send one aggregated reduction to tile_hist[digit][tile]; the table is zero on entry
-        if (WRITE_KEYS && tile_hist) {
-            const uint32_t d = (p < np) ? (key & digit_mask) : 0xffffffffu;
-            const uint32_t peers = __match_any_sync(0xffffffffu, d);
-            if (p < np && lane == __ffs(peers) - 1)
-                atomicAdd(&tile_hist[(size_t)d * ntiles + (size_t)(p0 / SORT_TILE)], (uint32_t)__popc(peers));
-        }
+        if (WRITE_KEYS && tile_hist) sw_hist(tile_hist, ntiles, p0 / SORT_TILE, valid, key, digit_mask, lane);
     }
 }
 
@@ -147,7 +167,7 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
     P.k0 = (uint32_t)q.seed; P.k1 = (uint32_t)(q.seed >> 32);
     P.step_lo = (uint32_t)step; P.step_hi = (uint32_t)(step >> 32);
     const int threads = 256;
-    int64_t want = (np + threads - 1) / threads;
+    const int64_t want = (np + threads - 1) / threads;
     const int64_t cap = (int64_t)ctx->num_sms * 16;
     const int blocks = (int)(want < cap ? want : cap);
     if (keys_out) {

@@ -123,6 +123,35 @@ def test_stream_walls(gpu, wl, orc, name):
     ctx.close()
 
 
+def test_stream_walls_unaligned(gpu, wl, orc):
+    """Array views that start 4 bytes past a 16-byte boundary and a particle count that is not a multiple of 4
+    (nor of the warp size) must give the same bits as aligned arrays."""
+    import torch
+    cfg, st = wl.cavity(n=16, ppc=37, seed=9)
+    cfg = dict(cfg, dt=float(np.float32(0.03)))
+    keep = st["x"].shape[0] - 3                     # 9469 particles: not a multiple of 4
+    st = {k: v[:keep].copy() for k, v in st.items()}
+    ref = orc.stream_walls(st, cfg, 5)
+    ctx = gpu.Context(cfg)
+    for off in (0, 1):
+        d = {}
+        for k, v in st.items():
+            buf = torch.empty(keep + 4, dtype=torch.int32 if k == "pid" else torch.float32, device="cuda")
+            d[k] = buf[off:off + keep]
+            d[k].copy_(torch.from_numpy(v.view(np.int32) if k == "pid" else v))
+        ctx.stream_walls(d, 5)
+        got = {k: v.cpu().numpy() for k, v in d.items()}
+        assert np.array_equal(_bits(got["x"]), _bits(ref["x"])), off
+        assert np.array_equal(_bits(got["y"]), _bits(ref["y"])), off
+        hit = (_bits(ref["vx"]) != _bits(st["vx"])) | (_bits(ref["vy"]) != _bits(st["vy"])) | (_bits(ref["vz"]) != _bits(st["vz"]))
+        assert hit.sum() > 0
+        for k in ("vx", "vy", "vz"):
+            assert np.array_equal(_bits(got[k])[~hit], _bits(st[k])[~hit])
+            allowed = 1e-6 * np.maximum(np.abs(ref[k][hit].astype(np.float64)), np.sqrt(0.5))
+            assert (np.abs(got[k][hit].astype(np.float64) - ref[k][hit]) <= allowed).all(), (off, k)
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------------ a7 fp_step
 def _one_step(gpu, orc, cfg, st, closure, mlp, step_no, tau_fn=None, tau_ref_n=0.0):
     import torch
