@@ -223,6 +223,7 @@ def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
         res["closure_mlp"] = timed(lambda r: fpcl.fp_closure_mlp(ctx.h, mom_lite, 13, None, mlp_dev, 1.0, coef, flags),
                                    "closure_mlp")
         res["closure_mlp"]["cells_per_s"] = ncell / (res["closure_mlp"]["ms"] * 1e-3)
+        res["closure_mlp"]["kernel"] = "mma.sync TF32 with 3xTF32 compensation (default, ~1e-5)"
     fpcl.fp_closure_exact(ctx.h, mom_full, None, coef, flags)
     # the update rewrites velocities in place: each timed launch advances the same ensemble one collision step
     ts = []

@@ -132,7 +132,8 @@ int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell 
 
 /* a5 -- fused MLP surrogate: features -> standardise -> dense layers -> de-standardise (PAPER.md:264, :309,
  * :327).  mom_stride 13 or 29.  relax_w in (0,1]: coef <- w*new + (1-w)*old; 1 overwrites.
- * Parameters are uploaded to context scratch when h_mlp's pointers/shape change (cached between calls). */
+ * The caller's weights (device memory, row-major [out][in]) are re-packed into context scratch by a small
+ * kernel on every call, on the same stream: weights changed in place between calls are always picked up. */
 int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell /* nullable */,
                    const fp_mlp* h_mlp, float relax_w, float* coef, uint32_t* flags, void* stream);
 

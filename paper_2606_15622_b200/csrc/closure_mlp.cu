@@ -8,7 +8,7 @@
 // (13-64-64-64-9: 39 KB), otherwise read through L1/L2.  Each thread produces 8 outputs per sweep over the
 // inputs, so one activation load and two broadcast 128-bit weight loads feed 8 FMAs.  Plain fp32 FMA pipe
 // (tolerance 1e-5); no tensor cores in this kernel.
-#include "common.cuh"
+#include "tiles.cuh"
 #include "upd_prep.cuh"
 
 #define MLP_OB 8
