@@ -263,19 +263,24 @@ def corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, steps):
         a = fpcl.to_device(st)
         b = {k: torch.empty_like(v) for k, v in a.items()}
         out = ctx.alloc_step_outputs(0)
+        # C5 has no inflow/outflow model (out of scope): its particles drift out of the analytic bow-shock field and
+        # pile up in the clamped outflow column, so it is timed over a few steps close to the designed 5..400 ppc
+        warm, steps_here = (10, steps) if name == "c4_8m" else (2, min(steps, 6))
         n = 0
-        for _ in range(10):
+        for _ in range(warm):
             ctx.step(a, b, n, out, closure=0, **kw); a, b = b, a; n += 1
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        for _ in range(steps):
+        for _ in range(steps_here):
             ctx.step(a, b, n, out, closure=0, **kw); a, b = b, a; n += 1
         e1.record(); e1.synchronize()
         np_ = a["x"].numel()
-        ms = e0.elapsed_time(e1) / steps
+        ms = e0.elapsed_time(e1) / steps_here
         tab = cold_kernel_table(fpcl, torch, ctx, a, out, mlp_dev, hbm_peak, reps=8)
-        res[name] = {"workload": label, "particles": np_, "cells": ctx.ncell, "fp_step_ms": ms,
+        counts = (out["cell_start"][1:] - out["cell_start"][:-1])
+        res[name] = {"workload": label, "particles": np_, "cells": ctx.ncell, "fp_step_ms": ms, "steps": steps_here,
+                     "max_particles_per_cell": int(counts.max().item()),
                      "particle_steps_per_s": np_ / (ms * 1e-3),
                      "flags_nonzero_cells": int((out["flags"] != 0).sum().item()), "kernels_cold_l2": tab}
         ctx.close()

@@ -15,8 +15,12 @@
 #ifndef FPW_G8_MIN
 #define FPW_G8_MIN 56.0            // 8 cells x 56 = 448
 #endif
+#ifndef FPW_G16_MIN
 #define FPW_G16_MIN 112.0          // 4 cells x 112 = 448
+#endif
+#ifndef FPW_G32_MIN
 #define FPW_G32_MIN 224.0          // 2 cells x 224 = 448
+#endif
 
 #ifdef __CUDACC__
 
