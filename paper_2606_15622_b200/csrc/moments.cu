@@ -165,6 +165,73 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     }
 }
 
+// A cell that alone exceeds the staging buffer (or unaligned arrays), all 32 lanes: both passes run over slices of the
+// cell copied to shared memory with plain coalesced loads (16 independent loads per lane and array in flight; any
+// alignment).  Per slice a lane adds at most MOM_CAP / 32 terms in fp32; slices are combined in fp64 (pass 1 per
+// lane, pass 2 after the transposing tree, lane i owning record slot i).  Twice the algorithmic traffic, no
+// per-iteration latency chain.
+template <bool FULL>
+__device__ __noinline__ void mom_giant_cell(const float* __restrict__ vx, const float* __restrict__ vy,
+                                            const float* __restrict__ vz, int32_t s, int32_t n, float* sx, int lane,
+                                            double* __restrict__ rec)
+{
+    constexpr int NREC = FULL ? 29 : 13;
+    float* sy = sx + MOM_CAP;
+    float* sz = sy + MOM_CAP;
+    const float px = vx[s], py = vy[s], pz = vz[s];                      // pivot: the cell's first particle
+    double S0 = 0.0, S1 = 0.0, S2 = 0.0;
+#pragma unroll 1
+    for (int32_t off = 0; off < n; off += MOM_CAP) {
+        const int32_t len = min((int32_t)MOM_CAP, n - off), b0 = s + off;
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+#pragma unroll 4
+        for (int32_t i = lane; i < len; i += 32) { a0 += vx[b0 + i] - px; a1 += vy[b0 + i] - py; a2 += vz[b0 + i] - pz; }
+        S0 += (double)a0; S1 += (double)a1; S2 += (double)a2;
+    }
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) { S0 += fpd_shfl_xor(S0, d); S1 += fpd_shfl_xor(S1, d); S2 += fpd_shfl_xor(S2, d); }
+    const double invn = 1.0 / (double)n;
+    const double m0d = S0 * invn, m1d = S1 * invn, m2d = S2 * invn;
+    const float m0 = (float)m0d, m1 = (float)m1d, m2 = (float)m2d;
+    double tot = 0.0;                                                     // lane i: record slot i
+#pragma unroll 1
+    for (int32_t off = 0; off < n; off += MOM_CAP) {
+        const int32_t len = min((int32_t)MOM_CAP, n - off), b0 = s + off;
+        __syncwarp();
+        for (int32_t i = lane; i < len; i += 32) { sx[i] = vx[b0 + i]; sy[i] = vy[b0 + i]; sz[i] = vz[b0 + i]; }
+        __syncwarp();
+        float r[32];
+#pragma unroll
+        for (int q = 0; q < 32; ++q) r[q] = 0.f;
+        for (int32_t i = lane; i < len; i += 32) {
+            const float cx = (sx[i] - px) - m0, cy = (sy[i] - py) - m1, cz = (sz[i] - pz) - m2;
+            const float xx = cx * cx, xy = cx * cy, xz = cx * cz, yy = cy * cy, yz = cy * cz, zz = cz * cz;
+            const float c2 = (xx + yy) + zz;
+            r[4] += xx; r[5] += xy; r[6] += xz; r[7] += yy; r[8] += yz; r[9] += zz;
+            if (FULL) {
+                r[10] = fmaf(xx, cx, r[10]); r[11] = fmaf(xx, cy, r[11]); r[12] = fmaf(xx, cz, r[12]);
+                r[13] = fmaf(xy, cy, r[13]); r[14] = fmaf(xy, cz, r[14]); r[15] = fmaf(xz, cz, r[15]);
+                r[16] = fmaf(yy, cy, r[16]); r[17] = fmaf(yy, cz, r[17]); r[18] = fmaf(yz, cz, r[18]);
+                r[19] = fmaf(zz, cz, r[19]);
+                r[20] = fmaf(c2, xx, r[20]); r[21] = fmaf(c2, xy, r[21]); r[22] = fmaf(c2, xz, r[22]);
+                r[23] = fmaf(c2, yy, r[23]); r[24] = fmaf(c2, yz, r[24]); r[25] = fmaf(c2, zz, r[25]);
+                const float c4 = c2 * c2;
+                r[26] = fmaf(c4, cx, r[26]); r[27] = fmaf(c4, cy, r[27]); r[28] = fmaf(c4, cz, r[28]);
+            } else {
+                r[10] = fmaf(c2, cx, r[10]); r[11] = fmaf(c2, cy, r[11]); r[12] = fmaf(c2, cz, r[12]);   // h_i
+            }
+        }
+        fpd_transpose_reduce<32, 32, float>(r, lane);
+        tot += (double)r[0];
+    }
+    double val = tot * invn;
+    if (lane == 0) val = (double)n;
+    else if (lane == 1) val = (double)px + m0d;
+    else if (lane == 2) val = (double)py + m1d;
+    else if (lane == 3) val = (double)pz + m2d;
+    if (lane < NREC) rec[lane] = val;
+}
+
 // The cells of a chunk that does not fit the staging buffer, one at a time: each staged on its own and reduced by
 // all 32 lanes; only a cell that alone exceeds the buffer reads global memory.  Kept out of line so that its
 // registers do not add to the common path's.
@@ -201,7 +268,8 @@ __device__ __noinline__ void mom_dense_chunk(const float* __restrict__ vx, const
             __syncwarp();
             mom_cell_group<32, FULL, true>(sx - rc.a0, sy - rc.a0, sz - rc.a0, s1c, e1c - s1c, true, lane, recc);
         } else {
-            mom_cell_group<32, FULL, false>(vx, vy, vz, s1c, e1c - s1c, true, lane, recc);
+            if (e1c > s1c) mom_giant_cell<FULL>(vx, vy, vz, s1c, e1c - s1c, sx, lane, recc);
+            else if (lane < NREC) recc[lane] = 0.0;                       // empty cell: N = 0 and zeros
         }
     }
 }
@@ -209,8 +277,11 @@ __device__ __noinline__ void mom_dense_chunk(const float* __restrict__ vx, const
 // Persistent warps: a warp owns chunks wg, wg + nwarps, ... of 32/G consecutive cells; while it reduces one chunk the
 // bulk copies of its next chunk are already in flight into the warp's other staging buffer (2-stage pipeline per
 // warp, mbarrier per stage), and the cell boundaries of the chunk after that are being fetched.
+#ifndef MOM_MINB
+#define MOM_MINB 4                      // 128 registers: four CTAs per SM is what the staging buffers allow
+#endif
 template <int G, bool FULL>
-__global__ void __launch_bounds__(MOM_THREADS)
+__global__ void __launch_bounds__(MOM_THREADS, MOM_MINB)
 moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
                     const int32_t* __restrict__ cell_start, int32_t ncell, int64_t np, int32_t aligned,
                     double* __restrict__ mom)
