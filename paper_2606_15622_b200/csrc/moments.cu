@@ -2,7 +2,7 @@
 // (PAPER.md:124 moment definition, :215-216 M1-M5, :243 LITE, :181 plain 1/N mean; R0).
 //
 // HBM-bound by design: 12 B/particle read once + one record per cell written.
-// A group of G lanes (G = 4/8/16 by mean particles per cell) owns one cell, so a warp works on 32/G consecutive cells
+// A group of G lanes (G = 4/8/16/32 by mean particles per cell, tiles.cuh) owns one cell, so a warp works on 32/G consecutive cells
 // at once.  Each warp stages the contiguous vx, vy, vz slices of its cells in its own shared-memory buffer with three
 // 1D bulk asynchronous copies (tiles.cuh) -- HBM is read once, coalesced, with no block-wide barrier and no
 // dependence between warps -- and both passes over a cell read shared memory:
@@ -12,8 +12,10 @@
 //   pass 2: c = (v - v_pivot) - m in fp32, monomials and per-lane partial sums in fp32 (<= 64 terms per lane and
 //           chunk), combined across the group by a balanced fp32 tree (a transposing butterfly that leaves record
 //           slot k in the lane that stores it); chunks, the mean and the 1/N normalisation are fp64.
-// Cells larger than G*64 particles are processed chunk by chunk with fp64 accumulation between chunks.  A warp whose
-// cells do not fit its staging buffer (dense or huge cells), or unaligned arrays, run the same code on global pointers.
+// A chunk whose cells do not fit the warp's staging buffer (load-imbalanced grids) is walked cell by cell, each cell
+// staged on its own and reduced by all 32 lanes; a cell that alone exceeds the buffer, and unaligned arrays, take
+// mom_giant_cell: the same two passes over shared-memory slices filled by plain coalesced loads, slices combined in
+// fp64.
 #include "tiles.cuh"
 
 #ifndef MOM_THREADS
@@ -25,9 +27,9 @@
 #define MOM_CAP FPW_CAP            // staged elements per array, warp and stage
 #endif
 
-// One cell per group of G lanes.  bx/by/bz may point to shared or global memory; particle p is at b?[p].
-// INPLACE: the arrays are the warp's private staging copy, pass 1 overwrites v by v - v_pivot.
-template <int G, bool FULL, bool INPLACE>
+// One cell per group of G lanes.  bx/by/bz: the warp's private staging copy in shared memory, particle p at b?[p];
+// pass 1 overwrites v by v - v_pivot.
+template <int G, bool FULL>
 __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,
                                                bool have, int gl, double* __restrict__ rec)
 {
@@ -54,15 +56,14 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
             const float2 w1 = fpd_add2(make_float2(by[s + j], by[s + j + G]), npy);
             const float2 w2 = fpd_add2(make_float2(bz[s + j], bz[s + j + G]), npz);
             A0 = fpd_add2(A0, w0); A1 = fpd_add2(A1, w1); A2 = fpd_add2(A2, w2);
-            if (INPLACE) {      // park w = v - v_pivot for pass 2 (store pipe is idle, the FMA pipe is the bottleneck)
-                wx[s + j] = w0.x; wx[s + j + G] = w0.y; wy[s + j] = w1.x; wy[s + j + G] = w1.y;
-                wz[s + j] = w2.x; wz[s + j + G] = w2.y;
-            }
+            // park w = v - v_pivot for pass 2 (store pipe is idle, the FMA pipe is the bottleneck)
+            wx[s + j] = w0.x; wx[s + j + G] = w0.y; wy[s + j] = w1.x; wy[s + j + G] = w1.y;
+            wz[s + j] = w2.x; wz[s + j + G] = w2.y;
         }
         if (j < cend) {
             const float w0 = bx[s + j] - px, w1 = by[s + j] - py, w2 = bz[s + j] - pz;
             A0.x += w0; A1.x += w1; A2.x += w2;
-            if (INPLACE) { wx[s + j] = w0; wy[s + j] = w1; wz[s + j] = w2; }
+            wx[s + j] = w0; wy[s + j] = w1; wz[s + j] = w2;
         }
         const float a0 = A0.x + A0.y, a1 = A1.x + A1.y, a2 = A2.x + A2.y;
         S0 += (double)a0; S1 += (double)a1; S2 += (double)a2;
@@ -96,15 +97,9 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
             const bool two = j + G < cend;
             const int32_t jb = two ? j + G : j;                            // lone last particle: second half masked
             float2 cx, cy, cz;
-            if (INPLACE) {
-                cx = fpd_add2(make_float2(bx[s + j], bx[s + jb]), nm0);
-                cy = fpd_add2(make_float2(by[s + j], by[s + jb]), nm1);
-                cz = fpd_add2(make_float2(bz[s + j], bz[s + jb]), nm2);
-            } else {
-                cx = fpd_add2(fpd_add2(make_float2(bx[s + j], bx[s + jb]), npx), nm0);
-                cy = fpd_add2(fpd_add2(make_float2(by[s + j], by[s + jb]), npy), nm1);
-                cz = fpd_add2(fpd_add2(make_float2(bz[s + j], bz[s + jb]), npz), nm2);
-            }
+            cx = fpd_add2(make_float2(bx[s + j], bx[s + jb]), nm0);
+            cy = fpd_add2(make_float2(by[s + j], by[s + jb]), nm1);
+            cz = fpd_add2(make_float2(bz[s + j], bz[s + jb]), nm2);
             if (!two) { cx.y = 0.f; cy.y = 0.f; cz.y = 0.f; }
             const float2 xx = fpd_mul2(cx, cx), xy = fpd_mul2(cx, cy), xz = fpd_mul2(cx, cz);
             const float2 yy = fpd_mul2(cy, cy), yz = fpd_mul2(cy, cz), zz = fpd_mul2(cz, cz);
@@ -266,7 +261,7 @@ __device__ __noinline__ void mom_dense_chunk(const float* __restrict__ vx, const
             }
             if (bytes > 0) { fpt_mbar_wait(bar, (phase >> b) & 1u); phase ^= 1u << b; }
             __syncwarp();
-            mom_cell_group<32, FULL, true>(sx - rc.a0, sy - rc.a0, sz - rc.a0, s1c, e1c - s1c, true, lane, recc);
+            mom_cell_group<32, FULL>(sx - rc.a0, sy - rc.a0, sz - rc.a0, s1c, e1c - s1c, true, lane, recc);
         } else {
             if (e1c > s1c) mom_giant_cell<FULL>(vx, vy, vz, s1c, e1c - s1c, sx, lane, recc);
             else if (lane < NREC) recc[lane] = 0.0;                       // empty cell: N = 0 and zeros
@@ -348,7 +343,7 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
             }
             if (r_cur.nb > 0) { fpt_mbar_wait(&wbar[b], (phase >> b) & 1u); phase ^= 1u << b; }
             __syncwarp();
-            mom_cell_group<G, FULL, true>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, s, n, have, gl, rec);   // shared-memory loads
+            mom_cell_group<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, s, n, have, gl, rec);   // shared-memory loads
         } else {
             // a chunk too dense for the staging buffer (load-imbalanced grids): cell by cell in buffer b
             mom_dense_chunk<FULL>(vx, vy, vz, cs_cur, CPW, chunk, ncell, np, aligned, wbuf + (size_t)b * 3 * MOM_CAP,
