@@ -39,6 +39,7 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
     c->err[0] = 0;
     c->p = q;
     { const char* e = getenv("FPCL_MLP_FP32"); c->mlp_force_fp32 = e && e[0] == '1'; }
+    { const char* e = getenv("FPCL_SORT_UNPACKED"); c->sort_no_pack = e && e[0] == '1'; }
     c->ncell = q.nx * q.ny;
     int bits = 0;
     while (((int64_t)1 << bits) < (int64_t)c->ncell) ++bits;

@@ -6,7 +6,10 @@
 // of a pass is produced by whoever writes that pass's input (key_kernel / the stream kernel for the first pass, the
 // previous scatter for the later ones), hist_kernel only serves callers that bring their own keys.  Stability
 // inside a tile comes from warp-striped item order plus __match_any_sync ranking (no atomics decide an order).
-// The payload (x, y, vx, vy, vz, pid) is gathered once at the end through the final permutation.
+// The payload (x, y, vx, vy, vz, pid) is gathered once at the end through the final permutation.  Two-pass sorts whose
+// index and high digit fit one 32-bit word (4M particles x 40k cells: 22 + 8 bits) move that single word between the
+// passes instead of a key and an index, and do not store sorted keys at all (the gather recomputes a particle's key
+// from the positions it reads anyway): 16 B/particle less traffic and one register array less in the scatter.
 #include "common.cuh"
 
 // cell keys of tile blockIdx.x plus the tile's histogram of the first radix digit
@@ -87,26 +90,34 @@ scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_t
 
 __device__ __forceinline__ int dbits_of(int bins) { return 31 - __clz(bins); }
 
+// What a scatter pass reads and writes.  PLAIN: (key, index) pairs in two arrays.  With two passes and
+// index bits + high-digit bits <= 32 the pair travels as one word between the passes: PACK_OUT (first pass) writes
+// (high digit << pack_bits) | index into keys_out, PACK_IN (second pass) reads that word, ranks by its digit and
+// writes only the index; the sorted keys are not stored (the gather recomputes them from the positions).
+enum { SORT_FIRST = 0, SORT_LATER = 1, SORT_PACK_OUT = 2, SORT_PACK_IN = 3 };
+
 // The items of one tile: load, rank, scatter.  FULLT: every item of the tile exists (no bounds checks).
-template <bool FIRST_PASS, bool FULLT>
+template <int MODE, bool FULLT>
 __device__ __forceinline__ void scatter_items(int64_t np, const uint32_t* __restrict__ keys_in,
                                               const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ keys_out,
                                               uint32_t* __restrict__ idx_out, int nblocks, int shift, int bins,
-                                              uint32_t* __restrict__ next_hist, uint32_t (*cnt)[SORT_MAX_BINS],
-                                              const uint32_t* bin_base)
+                                              int pack_bits, uint32_t* __restrict__ next_hist,
+                                              uint32_t (*cnt)[SORT_MAX_BINS], const uint32_t* bin_base)
 {
+    constexpr bool FIRST_PASS = (MODE == SORT_FIRST || MODE == SORT_PACK_OUT);
+    constexpr bool HAS_IDX = (MODE == SORT_LATER);       // a separate index array comes in
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t mask = (uint32_t)bins - 1u;
     const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS) + lane;   // this lane's first item
     const uint32_t* kp = keys_in + wbase;
-    const uint32_t* ip = FIRST_PASS ? nullptr : idx_in + wbase;
-    uint32_t key[SORT_ITEMS], idx[SORT_ITEMS], rank[SORT_ITEMS];
+    const uint32_t* ip = HAS_IDX ? idx_in + wbase : nullptr;
+    uint32_t key[SORT_ITEMS], idx[SORT_ITEMS], rank[SORT_ITEMS];   // PACK_IN: key[] holds the packed word, idx[] is unused
     bool valid[SORT_ITEMS];
 #pragma unroll
     for (int i = 0; i < SORT_ITEMS; ++i) {
         valid[i] = FULLT ? true : (wbase + i * 32 < np);
         key[i] = valid[i] ? kp[i * 32] : 0xffffffffu;
-        idx[i] = FIRST_PASS ? (uint32_t)wbase + (uint32_t)(i * 32) : (valid[i] ? ip[i * 32] : 0u);
+        idx[i] = FIRST_PASS ? (uint32_t)wbase + (uint32_t)(i * 32) : ((HAS_IDX && valid[i]) ? ip[i * 32] : 0u);
     }
     // rank inside the warp's sub-tile, round by round (stable)
 #pragma unroll
@@ -140,8 +151,9 @@ __device__ __forceinline__ void scatter_items(int64_t np, const uint32_t* __rest
         if (valid[i]) {
             const uint32_t d = (key[i] >> shift) & mask;
             const uint32_t dst = bin_base[d] + cnt[warp][d] + rank[i];
-            keys_out[dst] = key[i];
-            idx_out[dst] = idx[i];
+            if (MODE == SORT_PACK_OUT) keys_out[dst] = ((key[i] >> (shift + dbits_of(bins))) << pack_bits) | idx[i];
+            else if (MODE == SORT_PACK_IN) idx_out[dst] = key[i] & ((1u << pack_bits) - 1u);
+            else { keys_out[dst] = key[i]; idx_out[dst] = idx[i]; }
             code = (((key[i] >> shift) >> dbits_of(bins)) & mask) << 20 | (dst / SORT_TILE);
         }
         // the next pass's tile histograms: the tile an item lands in is known here, so lanes that agree on
@@ -159,12 +171,12 @@ __device__ __forceinline__ void scatter_items(int64_t np, const uint32_t* __rest
 #ifndef SORT_SCATTER_MINB
 #define SORT_SCATTER_MINB 4                               // 64 registers: four tiles per SM hide the latency phases
 #endif
-template <bool FIRST_PASS>
+template <int MODE>
 __global__ void __launch_bounds__(SORT_THREADS, SORT_SCATTER_MINB)
 scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
                uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out,
                const uint32_t* __restrict__ block_hist, const uint32_t* __restrict__ bin_total, int nblocks,
-               int shift, int bins, uint32_t* __restrict__ next_hist)
+               int shift, int bins, int pack_bits, uint32_t* __restrict__ next_hist)
 {
     fpd_pdl();
     __shared__ uint32_t cnt[SORT_WARPS][SORT_MAX_BINS];   // per-warp running digit counts, then bases
@@ -197,30 +209,65 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
     }
     __syncthreads();
     if ((int64_t)(blockIdx.x + 1) * SORT_TILE <= np)       // block-uniform: all but the last tile are full
-        scatter_items<FIRST_PASS, true>(np, keys_in, idx_in, keys_out, idx_out, nblocks, shift, bins, next_hist, cnt, bin_base);
+        scatter_items<MODE, true>(np, keys_in, idx_in, keys_out, idx_out, nblocks, shift, bins, pack_bits, next_hist, cnt, bin_base);
     else
-        scatter_items<FIRST_PASS, false>(np, keys_in, idx_in, keys_out, idx_out, nblocks, shift, bins, next_hist, cnt, bin_base);
+        scatter_items<MODE, false>(np, keys_in, idx_in, keys_out, idx_out, nblocks, shift, bins, pack_bits, next_hist, cnt, bin_base);
 }
 
 // payload permute fused with cell_start from the sorted keys: cell_start[k] = first position whose key >= k,
 // cell_start[ncell] = np.  Thread k owns the boundary between positions k-1 and k (and the last one also np).
+// FROM_POS (packed sort): the sorted keys were not stored; a particle's key is recomputed from the positions this
+// kernel gathers anyway (the same function of the same numbers as the key that was sorted), the left neighbour's
+// key comes from the lane below or, for lane 0, from the neighbour's positions.
+struct gather_grid { int32_t nx, ny; float x0, y0, inv_dx, inv_dy; };
+
+template <bool FROM_POS>
 __global__ void __launch_bounds__(256)
 gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ skeys, int32_t ncell,
               int32_t* __restrict__ cell_start,
               const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ vx,
               const float* __restrict__ vy, const float* __restrict__ vz, const uint32_t* __restrict__ pid,
               float* __restrict__ xo, float* __restrict__ yo, float* __restrict__ vxo, float* __restrict__ vyo,
-              float* __restrict__ vzo, uint32_t* __restrict__ pido)
+              float* __restrict__ vzo, uint32_t* __restrict__ pido, const __grid_constant__ gather_grid Gd)
 {
     fpd_pdl();
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < np; k += stride) {
-        const uint32_t s = perm[k];
-        const uint32_t key = skeys[k];
-        const int64_t lo = (k == 0) ? 0 : (int64_t)skeys[k - 1] + 1;
-        xo[k] = x[s]; yo[k] = y[s]; vxo[k] = vx[s]; vyo[k] = vy[s]; vzo[k] = vz[s]; pido[k] = pid[s];
-        for (int64_t c = lo; c <= (int64_t)key; ++c) cell_start[c] = (int32_t)k;
-        if (k == np - 1) for (int64_t c = (int64_t)key + 1; c <= (int64_t)ncell; ++c) cell_start[c] = (int32_t)np;
+    const int lane = threadIdx.x & 31;
+    for (int64_t k0 = (int64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31); k0 < np; k0 += stride) {   // warp-uniform
+        const int64_t k = k0 + lane;
+        const bool valid = k < np;
+        uint32_t key = 0;
+        float px = 0.f, py = 0.f;
+        uint32_t s = 0;
+        if (valid) {
+            s = perm[k];
+            px = x[s]; py = y[s];
+            if (FROM_POS) {
+                const int32_t ix = fpd_axis_index(px, Gd.x0, Gd.inv_dx, Gd.nx);
+                const int32_t iy = (Gd.ny > 1) ? fpd_axis_index(py, Gd.y0, Gd.inv_dy, Gd.ny) : 0;
+                key = (uint32_t)(iy * Gd.nx + ix);
+            } else {
+                key = skeys[k];
+            }
+        }
+        int64_t lo = 0;
+        if (FROM_POS) {
+            uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+            if (valid && lane == 0 && k > 0) {
+                const uint32_t s2 = perm[k - 1];
+                const int32_t ix = fpd_axis_index(x[s2], Gd.x0, Gd.inv_dx, Gd.nx);
+                const int32_t iy = (Gd.ny > 1) ? fpd_axis_index(y[s2], Gd.y0, Gd.inv_dy, Gd.ny) : 0;
+                prev = (uint32_t)(iy * Gd.nx + ix);
+            }
+            lo = (k == 0) ? 0 : (int64_t)prev + 1;
+        } else if (valid) {
+            lo = (k == 0) ? 0 : (int64_t)skeys[k - 1] + 1;
+        }
+        if (valid) {
+            xo[k] = px; yo[k] = py; vxo[k] = vx[s]; vyo[k] = vy[s]; vzo[k] = vz[s]; pido[k] = pid[s];
+            for (int64_t c = lo; c <= (int64_t)key; ++c) cell_start[c] = (int32_t)k;
+            if (k == np - 1) for (int64_t c = (int64_t)key + 1; c <= (int64_t)ncell; ++c) cell_start[c] = (int32_t)np;
+        }
     }
 }
 
@@ -256,6 +303,10 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     const int dbits = fpi_sort_digit_bits(ctx);
     const int bins = 1 << dbits;
     if ((size_t)bins * nblocks > ctx->block_hist_elems) return fp_fail(ctx, FP_ERR_STATE, "sort scratch too small");
+    // two passes and (index, high digit) fit one word: the pair travels packed between the passes
+    int idx_bits = 1;
+    while (idx_bits < 32 && ((int64_t)1 << idx_bits) < np) ++idx_bits;
+    const bool packed = !ctx->sort_no_pack && passes == 2 && idx_bits + (bits - dbits) <= 32;
     const uint32_t* kin = keys;
     const uint32_t* iin = nullptr;
     uint32_t* kout = ctx->key_a;
@@ -270,10 +321,14 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
         }
         fp_launch(scan_rows_kernel, bins, 256, 0, st, table, ctx->bin_total, nblocks, other);
         uint32_t* next = (pass + 1 < passes) ? other : nullptr;
-        if (pass == 0)
-            fp_launch(scatter_kernel<true>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
+        if (packed && pass == 0)
+            fp_launch(scatter_kernel<SORT_PACK_OUT>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, idx_bits, next);
+        else if (packed)                              // the digit sits above the index bits of the packed word
+            fp_launch(scatter_kernel<SORT_PACK_IN>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, idx_bits, bins, idx_bits, next);
+        else if (pass == 0)
+            fp_launch(scatter_kernel<SORT_FIRST>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, 0, next);
         else
-            fp_launch(scatter_kernel<false>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, next);
+            fp_launch(scatter_kernel<SORT_LATER>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, 0, next);
         FP_LAUNCH_OK(ctx);
         FP_COUNT(ctx, 2);
         kin = kout; iin = iout;
@@ -284,8 +339,15 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     fp_mark(ctx, 2, st);
     const int64_t cap = (int64_t)ctx->num_sms * 16;
     const int64_t want = (np + 255) / 256;
-    fp_launch(gather_kernel, (int)(want < cap ? want : cap), 256, 0, st, np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
-                                                                 x_out, y_out, vx_out, vy_out, vz_out, pid_out);
+    const int gblocks = (int)(want < cap ? want : cap);
+    gather_grid Gd;
+    Gd.nx = ctx->p.nx; Gd.ny = ctx->p.ny; Gd.x0 = ctx->p.x0; Gd.y0 = ctx->p.y0; Gd.inv_dx = ctx->inv_dx; Gd.inv_dy = ctx->inv_dy;
+    if (packed)
+        fp_launch(gather_kernel<true>, gblocks, 256, 0, st, np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
+                  x_out, y_out, vx_out, vy_out, vz_out, pid_out, Gd);
+    else
+        fp_launch(gather_kernel<false>, gblocks, 256, 0, st, np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
+                  x_out, y_out, vx_out, vy_out, vz_out, pid_out, Gd);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
     if (perm) FP_CUDA_OK(ctx, cudaMemcpyAsync(perm, iin, (size_t)np * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));

@@ -76,6 +76,23 @@ def test_sort_edge_positions(gpu, wl, orc):
     ctx.close()
 
 
+def test_sort_two_array_path(gpu, wl, orc, monkeypatch):
+    """Two-pass sorts normally carry (high digit, index) as one packed word between the passes; ensembles too large
+    for that (index bits + digit bits > 32, e.g. the 20M-particle cylinder case) move keys and indices as two arrays.
+    FPCL_SORT_UNPACKED=1 forces that path at a size the oracle sorts in a blink."""
+    import torch
+    monkeypatch.setenv("FPCL_SORT_UNPACKED", "1")
+    cfg, st = wl.ragged(nx=41, ny=29, seed=23, mean_ppc=25.0)
+    ref, cs, perm = orc.sort_by_cell(st, cfg)
+    ctx = gpu.Context(cfg)
+    out, csd, pd = ctx.sort_by_cell(gpu.to_device(st), want_perm=True)
+    assert np.array_equal(csd.cpu().numpy(), cs)
+    assert np.array_equal(pd.cpu().numpy().view(np.uint32), perm)
+    for k in ("x", "y", "vx", "vy", "vz", "pid"):
+        assert np.array_equal(out[k].cpu().numpy().view(np.uint32), np.ascontiguousarray(ref[k]).view(np.uint32)), k
+    ctx.close()
+
+
 def test_sort_three_passes(gpu, wl, orc):
     """More than 2^18 cells forces a third radix pass."""
     rng = np.random.default_rng(5)
