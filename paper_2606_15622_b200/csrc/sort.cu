@@ -231,12 +231,13 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
               float* __restrict__ vzo, uint32_t* __restrict__ pido, const __grid_constant__ gather_grid Gd)
 {
     fpd_pdl();
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    // cell_start is int32, so np < 2^31 and every index fits 32 bits
+    const int n = (int)np, stride = (int)(gridDim.x * blockDim.x);
     const int lane = threadIdx.x & 31;
-    for (int64_t k0 = (int64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31); k0 < np; k0 += stride) {   // warp-uniform
-        const int64_t k = k0 + lane;
-        const bool valid = k < np;
-        uint32_t key = 0;
+    for (int k0 = (int)(blockIdx.x * blockDim.x + (threadIdx.x & ~31)); k0 < n; k0 += stride) {   // warp-uniform
+        const int k = k0 + lane;
+        const bool valid = k < n;
+        int key = 0, lo = 0;
         float px = 0.f, py = 0.f;
         uint32_t s = 0;
         if (valid) {
@@ -245,28 +246,26 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
             if (FROM_POS) {
                 const int32_t ix = fpd_axis_index(px, Gd.x0, Gd.inv_dx, Gd.nx);
                 const int32_t iy = (Gd.ny > 1) ? fpd_axis_index(py, Gd.y0, Gd.inv_dy, Gd.ny) : 0;
-                key = (uint32_t)(iy * Gd.nx + ix);
+                key = iy * Gd.nx + ix;
             } else {
-                key = skeys[k];
+                key = (int)skeys[k];
+                lo = (k == 0) ? 0 : (int)skeys[k - 1] + 1;
             }
         }
-        int64_t lo = 0;
         if (FROM_POS) {
-            uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
-            if (valid && lane == 0 && k > 0) {
+            int prev = __shfl_up_sync(0xffffffffu, key, 1);
+            if (lane == 0 && k > 0 && valid) {
                 const uint32_t s2 = perm[k - 1];
                 const int32_t ix = fpd_axis_index(x[s2], Gd.x0, Gd.inv_dx, Gd.nx);
                 const int32_t iy = (Gd.ny > 1) ? fpd_axis_index(y[s2], Gd.y0, Gd.inv_dy, Gd.ny) : 0;
-                prev = (uint32_t)(iy * Gd.nx + ix);
+                prev = iy * Gd.nx + ix;
             }
-            lo = (k == 0) ? 0 : (int64_t)prev + 1;
-        } else if (valid) {
-            lo = (k == 0) ? 0 : (int64_t)skeys[k - 1] + 1;
+            lo = (k == 0) ? 0 : prev + 1;
         }
         if (valid) {
             xo[k] = px; yo[k] = py; vxo[k] = vx[s]; vyo[k] = vy[s]; vzo[k] = vz[s]; pido[k] = pid[s];
-            for (int64_t c = lo; c <= (int64_t)key; ++c) cell_start[c] = (int32_t)k;
-            if (k == np - 1) for (int64_t c = (int64_t)key + 1; c <= (int64_t)ncell; ++c) cell_start[c] = (int32_t)np;
+            for (int c = lo; c <= key; ++c) cell_start[c] = k;
+            if (k == n - 1) for (int c = key + 1; c <= ncell; ++c) cell_start[c] = n;
         }
     }
 }
