@@ -234,14 +234,16 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
     // cell_start is int32, so np < 2^31 and every index fits 32 bits
     const int n = (int)np, stride = (int)(gridDim.x * blockDim.x);
     const int lane = threadIdx.x & 31;
-    for (int k0 = (int)(blockIdx.x * blockDim.x + (threadIdx.x & ~31)); k0 < n; k0 += stride) {   // warp-uniform
+    const int kfirst = (int)(blockIdx.x * blockDim.x + (threadIdx.x & ~31));
+    uint32_t s_pref = (kfirst + lane < n) ? perm[kfirst + lane] : 0u;      // the permutation entry is fetched one trip ahead
+    for (int k0 = kfirst; k0 < n; k0 += stride) {                           // warp-uniform
         const int k = k0 + lane;
         const bool valid = k < n;
         int key = 0, lo = 0;
         float px = 0.f, py = 0.f;
-        uint32_t s = 0;
+        const uint32_t s = s_pref;
+        if ((int64_t)k + stride < n) s_pref = perm[k + stride];
         if (valid) {
-            s = perm[k];
             px = x[s]; py = y[s];
             if (FROM_POS) {
                 const int32_t ix = fpd_axis_index(px, Gd.x0, Gd.inv_dx, Gd.nx);
