@@ -153,9 +153,10 @@ def test_moments_mach10_shift(gpu, wl, orc):
 
 
 def test_moments_group_widths(gpu, wl, orc):
-    """Mean particles per cell selects the lane-group width (4, 8, 16): cover all three and one huge cell."""
+    """Mean particles per cell selects the lane-group width (4, 8, 16, 32): cover all four (the ragged counts also
+    send many chunks down the cell-by-cell and sliced paths) and one huge cell."""
     import torch
-    for mean_ppc, seed in ((12.0, 21), (90.0, 22), (260.0, 23)):
+    for mean_ppc, seed in ((12.0, 21), (90.0, 22), (150.0, 24), (260.0, 23)):
         cfg, st = wl.ragged(nx=16, ny=12, seed=seed, mean_ppc=mean_ppc)
         s, cs = _sorted_case(orc, cfg, st)
         ctx = gpu.Context(cfg)
