@@ -338,7 +338,13 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     }
     ctx->hist0_clean = (passes & 1) == 0;             // the last scan zeroed the table the last pass did not use
     fp_mark(ctx, 2, st);
-    const int64_t cap = (int64_t)ctx->num_sms * 16;
+    // one resident wave of grid-striding CTAs (a partial second wave costs 4 us at 4M particles)
+    static int gocc = 0;
+    if (gocc == 0) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&gocc, gather_kernel<true>, 256, 0);
+        if (gocc < 1) gocc = 1;
+    }
+    const int64_t cap = (int64_t)ctx->num_sms * gocc;
     const int64_t want = (np + 255) / 256;
     const int gblocks = (int)(want < cap ? want : cap);
     gather_grid Gd;

@@ -168,7 +168,13 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
     P.step_lo = (uint32_t)step; P.step_hi = (uint32_t)(step >> 32);
     const int threads = 256;
     const int64_t want = (np + threads - 1) / threads;
-    const int64_t cap = (int64_t)ctx->num_sms * 16;
+    // one resident wave of grid-striding CTAs (a partial extra wave costs up to 8 us at 4M particles)
+    static int socc = 0;
+    if (socc == 0) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&socc, sw_kernel<true>, threads, 0);
+        if (socc < 1) socc = 1;
+    }
+    const int64_t cap = (int64_t)ctx->num_sms * socc;
     const int blocks = (int)(want < cap ? want : cap);
     if (keys_out) {
         uint32_t* th = nullptr;
