@@ -12,7 +12,9 @@
 // radix sort tiling (sort.cu; the key kernel also produces the first digit histogram per tile)
 #define SORT_THREADS 256
 #define SORT_WARPS (SORT_THREADS / 32)
+#ifndef SORT_ITEMS
 #define SORT_ITEMS 16                                    // items per thread
+#endif
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)            // 4096 items per block
 #define SORT_MAX_BINS 512
 #define FPCL_NUM_SMS_DEFAULT 148

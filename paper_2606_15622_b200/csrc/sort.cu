@@ -73,8 +73,15 @@ scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_t
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int per = (nblocks + 255) / 256;
     const int beg = min(tid * per, nblocks), end = min(beg + per, nblocks);
+    constexpr int KEEP = 8;                       // counts held in registers (up to 2048 tiles = 8M particles) ...
+    uint32_t keep[KEEP];
     uint32_t sum = 0;
-    for (int i = beg; i < end; ++i) sum += row[i];
+    if (per <= KEEP) {
+#pragma unroll
+        for (int q = 0; q < KEEP; ++q) { keep[q] = (beg + q < end) ? row[beg + q] : 0u; sum += keep[q]; }
+    } else {                                      // ... re-read from global memory beyond that
+        for (int i = beg; i < end; ++i) sum += row[i];
+    }
     uint32_t incl = sum;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += t; }
@@ -84,7 +91,12 @@ scan_rows_kernel(uint32_t* __restrict__ block_hist, uint32_t* __restrict__ bin_t
 #pragma unroll
     for (int w = 0; w < 8; ++w) { if (w < warp) wbase += wsum[w]; total += wsum[w]; }
     uint32_t run = wbase + incl - sum;
-    for (int i = beg; i < end; ++i) { const uint32_t v = row[i]; row[i] = run; run += v; }
+    if (per <= KEEP) {
+#pragma unroll
+        for (int q = 0; q < KEEP; ++q) { if (beg + q < end) row[beg + q] = run; run += keep[q]; }
+    } else {
+        for (int i = beg; i < end; ++i) { const uint32_t v = row[i]; row[i] = run; run += v; }
+    }
     if (tid == 0) bin_total[blockIdx.x] = total;
 }
 
