@@ -245,6 +245,63 @@ def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
     return res
 
 
+def ppc_sweep(fpcl, torch, workloads, n_steps):
+    """BASELINE config 4: cavity Kn = 1.0, 200x200 cells, 20 / 50 / 200 particles per cell (seeds 40/41/42), n_steps
+    fp_steps with the exact closure.  Reports throughput and the conservation drift of the collision step: every
+    100th step the per-cell mean velocity and energy after the update (a second moment pass over the updated
+    velocities; the update moves no particle between cells) are compared with the moments the step itself took before
+    the update.  Scales: sqrt(theta) for the mean, 3 theta for the energy; cells the update skips are excluded."""
+    res = {}
+    for ppc, seed in ((20, 40), (50, 41), (200, 42)):
+        cfg, st = workloads.cavity(n=200, ppc=ppc, kn=1.0, seed=seed, shuffle=True)
+        ctx = fpcl.Context(cfg)
+        a = fpcl.to_device(st)
+        b = {k: torch.empty_like(v) for k, v in a.items()}
+        out = ctx.alloc_step_outputs(0)
+        np_ = a["x"].numel()
+        after = torch.empty((ctx.ncell, 13), dtype=torch.float64, device="cuda")
+        dmom, dene, flagged, nonfinite = 0.0, 0.0, 0, 0
+        energy = []
+        for w in range(5):
+            ctx.step(a, b, w, out, closure=0); a, b = b, a
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ms = 0.0
+        for blk in range(0, n_steps, 100):
+            nb = min(100, n_steps - blk)
+            e0.record()
+            for k in range(nb):
+                ctx.step(a, b, 5 + blk + k, out, closure=0); a, b = b, a
+            e1.record(); e1.synchronize()
+            ms += e0.elapsed_time(e1)
+            # drift of the last step of the block (a now holds its output)
+            ctx.cell_moments(a["vx"], a["vy"], a["vz"], out["cell_start"], 0, out=after)
+            before = out["mom"]
+            n = before[:, 0]
+            theta = (before[:, 4] + before[:, 7] + before[:, 9]) / 3.0
+            act = (n >= 2) & (theta > 0) & ((out["flags"] & 32) == 0)
+            if bool(act.any()):
+                du = (after[:, 1:4] - before[:, 1:4]).abs().amax(dim=1) / theta.clamp_min(1e-300).sqrt()
+                de = ((after[:, 4] + after[:, 7] + after[:, 9]) - 3.0 * theta).abs() / (3.0 * theta.clamp_min(1e-300))
+                dmom = max(dmom, float(du[act].max().item()))
+                dene = max(dene, float(de[act].max().item()))
+            flagged = max(flagged, int((out["flags"] != 0).sum().item()))
+            v2 = a["vx"].double() ** 2 + a["vy"].double() ** 2 + a["vz"].double() ** 2
+            nonfinite += int((~torch.isfinite(v2)).sum().item())
+            energy.append(float(v2.sum().item()) / np_)
+        res["ppc_%d" % ppc] = {"particles": np_, "steps": n_steps, "ms_per_step": ms / n_steps,
+                               "particle_steps_per_s": np_ * n_steps / (ms * 1e-3),
+                               "delta_particles": int(a["x"].numel() - np_),
+                               "collision_step_max_rel_momentum_change": dmom,
+                               "collision_step_max_rel_energy_change": dene,
+                               "max_flagged_cells": flagged, "nonfinite_velocities": nonfinite,
+                               "mean_v2_per_particle_every_100_steps": energy}
+        ctx.close()
+        del a, b, out, after
+        torch.cuda.empty_cache()
+    return res
+
+
 def corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, steps):
     """the judged kernels again where the velocity arrays cannot sit in the 126 MB L2 -- C4 at 200 ppc
     (8M particles, 96 MB of velocities) and C5 (hypersonic cylinder, ~20M particles, 5..400 per cell, 240 MB)."""
@@ -428,6 +485,7 @@ def main():
         if not args.small:
             del a2, b2, out2
             extras["beyond_l2"] = corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, min(args.steps, 20))
+            extras["c4_ppc_sweep"] = ppc_sweep(fpcl, torch, workloads, 1000 if args.steps >= 100 else 100)
 
     cpu_baseline = None
     if rank == 0 and not args.no_cpu_baseline:
