@@ -245,6 +245,29 @@ def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
     return res
 
 
+def closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak):
+    """BASELINE config 2: 100x100 cells x 50 particles from a Grad-13-perturbed Maxwellian (seed 1), no streaming:
+    moment gather, exact closure and surrogate timed separately (cold L2), flag counts and the condition estimates
+    of the exact closure (50 ppc makes some cells ill-conditioned by design)."""
+    cfg, st = workloads.grad13_cells()[:2]
+    ctx = fpcl.Context(cfg)
+    srt, cs, _ = ctx.sort_by_cell(fpcl.to_device(st), want_perm=False)
+    out = {"cell_start": cs}
+    tab = cold_kernel_table(fpcl, torch, ctx, srt, out, mlp_dev, hbm_peak, reps=20)
+    mom = ctx.cell_moments(srt["vx"], srt["vy"], srt["vz"], cs, 1)
+    coef, flags, kappa = ctx.closure_exact(mom, want_kappa=True)
+    kap = kappa.cpu().numpy()
+    fl = flags.cpu().numpy().view(np.uint32)
+    edges = [0.0, 1e2, 1e3, 1e4, 1e6, 1e8, float("inf")]
+    hist, _ = np.histogram(kap[kap > 0], bins=edges)
+    res = {"particles": int(srt["x"].numel()), "cells": ctx.ncell, "kernels_cold_l2": tab,
+           "flag_counts": {"illcond": int((fl & 8 != 0).sum()), "singular": int((fl & 4 != 0).sum()),
+                           "lowcount": int((fl & 2 != 0).sum()), "empty": int((fl & 1 != 0).sum())},
+           "kappa_estimate_histogram": {"edges": edges[:-1] + ["inf"], "counts": [int(c) for c in hist]}}
+    ctx.close()
+    return res
+
+
 def ppc_sweep(fpcl, torch, workloads, n_steps):
     """BASELINE config 4: cavity Kn = 1.0, 200x200 cells, 20 / 50 / 200 particles per cell (seeds 40/41/42), n_steps
     fp_steps with the exact closure.  Reports throughput and the conservation drift of the collision step: every
@@ -485,6 +508,7 @@ def main():
         if not args.small:
             del a2, b2, out2
             extras["beyond_l2"] = corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, min(args.steps, 20))
+            extras["c2_closure_microbench"] = closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak)
             extras["c4_ppc_sweep"] = ppc_sweep(fpcl, torch, workloads, 1000 if args.steps >= 100 else 100)
 
     cpu_baseline = None
