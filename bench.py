@@ -245,6 +245,33 @@ def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
     return res
 
 
+def couette_small(fpcl, torch, workloads):
+    """BASELINE config 1: 1D Couette, 50 cells x 100 particles, 100 fp_steps with the exact closure and again with the
+    13-64-64-64-9 SiLU surrogate.  At 5,000 particles a step is nine kernel launches' worth of latency."""
+    res = {}
+    cfg, st = workloads.couette()
+    mlp = fpcl.Mlp(workloads.xavier_mlp(n_scale=0.01, tau=cfg["tau"]))
+    for name, closure in (("exact", 0), ("mlp", 1)):
+        ctx = fpcl.Context(cfg)
+        a = fpcl.to_device(st)
+        b = {k: torch.empty_like(v) for k, v in a.items()}
+        out = ctx.alloc_step_outputs(closure)
+        for w in range(10):
+            ctx.step(a, b, w, out, closure=closure, mlp=mlp if closure else None); a, b = b, a
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for w in range(100):
+            ctx.step(a, b, 10 + w, out, closure=closure, mlp=mlp if closure else None); a, b = b, a
+        e1.record(); e1.synchronize()
+        ms = e0.elapsed_time(e1) / 100
+        res[name] = {"particles": int(a["x"].numel()), "cells": ctx.ncell, "ms_per_step": ms,
+                     "particle_steps_per_s": a["x"].numel() / (ms * 1e-3),
+                     "flagged_cells": int((out["flags"] != 0).sum().item())}
+        ctx.close()
+    return res
+
+
 def closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak):
     """BASELINE config 2: 100x100 cells x 50 particles from a Grad-13-perturbed Maxwellian (seed 1), no streaming:
     moment gather, exact closure and surrogate timed separately (cold L2), flag counts and the condition estimates
@@ -508,6 +535,7 @@ def main():
         if not args.small:
             del a2, b2, out2
             extras["beyond_l2"] = corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, min(args.steps, 20))
+            extras["c1_couette"] = couette_small(fpcl, torch, workloads)
             extras["c2_closure_microbench"] = closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak)
             extras["c4_ppc_sweep"] = ppc_sweep(fpcl, torch, workloads, 1000 if args.steps >= 100 else 100)
 
