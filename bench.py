@@ -506,9 +506,9 @@ def main():
     # dominant single kernel of the step (sort_keys is six launches; the others are one kernel each)
     single = {n: stages[n] for n in ("stream_walls", "gather", "moments", "closure", "update")}
     dom = max(single, key=lambda n: single[n]["ms"])
-    # DRAM traffic per launch from the committed ncu --set full capture (profiles/r01_ncu_full_v4.md, C3), bytes;
+    # DRAM traffic per launch from the committed ncu --set full capture (profiles/r01_ncu_full_v6.md, C3), bytes;
     # the in-place update's writes are still in L2 when its kernel ends, so its figure is mostly reads
-    ncu_traffic = {"update": 70.7e6, "moments": 48.4e6, "gather": 204.6e6, "stream_walls": 91.2e6,
+    ncu_traffic = {"update": 70.3e6, "moments": 48.4e6, "gather": 173.7e6, "stream_walls": 69.5e6,
                    "closure": 9.3e6 if closure == 0 else 4.3e6}
     roofline = {"kernel": dom, "bound": "hbm", "achieved": single[dom]["GBps_algorithmic"], "peak": hbm_peak,
                 "unit": "GB/s", "frac": single[dom]["frac_of_hbm_peak"],
