@@ -169,8 +169,10 @@ int fp_step(fp_ctx* ctx, int64_t np,
 
 /* Host-buffer convenience used by the end-to-end measurement: uploads the six SoA arrays from host memory
  * (pinned or pageable), runs fp_step on internally held device buffers sized max_particles, and downloads the
- * updated SoA plus cell_start, flags and coef back into the host arrays.  Synchronises the stream before
- * returning.  h_* are HOST pointers; h_coef [ncell*9], h_flags [ncell], h_cell_start [ncell+1]. */
+ * updated SoA plus cell_start, flags and coef back into the host arrays.  The upload of vz (needed only by the
+ * payload gather) and the download of x, y, pid (final after the gather) run on a context-owned side stream so that
+ * they overlap the kernels; both streams are synchronised before returning.
+ * h_* are HOST pointers; h_coef [ncell*9], h_flags [ncell], h_cell_start [ncell+1]. */
 int fp_step_host(fp_ctx* ctx, int64_t np,
                  float* h_x, float* h_y, float* h_vx, float* h_vy, float* h_vz, uint32_t* h_pid,
                  int32_t closure, const fp_mlp* h_mlp, float relax_w, uint64_t step,

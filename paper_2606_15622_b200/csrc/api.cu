@@ -19,6 +19,8 @@ static void fp_free_all(fp_ctx* c)
     cudaFree(c->block_hist); cudaFree(c->bin_total); cudaFree(c->cellc);
     for (int s = 0; s < 2; ++s) { for (int k = 0; k < 5; ++k) cudaFree(c->hs_f[s][k]); cudaFree(c->hs_pid[s]); }
     cudaFree(c->hs_mom); cudaFree(c->hs_coef); cudaFree(c->hs_flags); cudaFree(c->hs_cell_start);
+    if (c->hs_side) cudaStreamDestroy(c->hs_side);
+    for (int k = 0; k < 4; ++k) if (c->hs_ev[k]) cudaEventDestroy(c->hs_ev[k]);
     cudaFree(c->mlp.blob); cudaFree(c->mlp.tc_frags);
 }
 
@@ -201,6 +203,8 @@ static int fp_host_stage_alloc(fp_ctx* c)
     FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_coef, (size_t)c->ncell * 9 * 4));
     FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_flags, (size_t)c->ncell * 4));
     FP_CUDA_OK(c, cudaMalloc((void**)&c->hs_cell_start, ((size_t)c->ncell + 1) * 4));
+    FP_CUDA_OK(c, cudaStreamCreateWithFlags(&c->hs_side, cudaStreamNonBlocking));
+    for (int k = 0; k < 4; ++k) FP_CUDA_OK(c, cudaEventCreateWithFlags(&c->hs_ev[k], cudaEventDisableTiming));
     c->hs_ready = true;
     return FP_OK;
 }
@@ -218,18 +222,37 @@ extern "C" int fp_step_host(fp_ctx* ctx, int64_t np,
     cudaStream_t st = (cudaStream_t)stream;
     float* hp[5] = {h_x, h_y, h_vx, h_vy, h_vz};
     const size_t nb = (size_t)np * 4;
-    for (int k = 0; k < 5; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_f[0][k], hp[k], nb, cudaMemcpyHostToDevice, st));
+    cudaStream_t side = ctx->hs_side;
+    // host -> device: x, y, vx, vy, pid feed the stream kernel and the key sort; vz is needed only by the payload
+    // gather, so it travels on the side stream while those kernels run
+    FP_CUDA_OK(ctx, cudaEventRecord(ctx->hs_ev[0], st));                 // everything the caller queued before us
+    for (int k = 0; k < 4; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_f[0][k], hp[k], nb, cudaMemcpyHostToDevice, st));
     if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_pid[0], h_pid, nb, cudaMemcpyHostToDevice, st));
+    FP_CUDA_OK(ctx, cudaStreamWaitEvent(side, ctx->hs_ev[0], 0));
+    if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_f[0][4], hp[4], nb, cudaMemcpyHostToDevice, side));
+    FP_CUDA_OK(ctx, cudaEventRecord(ctx->hs_ev[1], side));
+    ctx->ev_before_gather = ctx->hs_ev[1];
+    ctx->ev_after_gather = ctx->hs_ev[2];
     rc = fp_step(ctx, np, ctx->hs_f[0][0], ctx->hs_f[0][1], ctx->hs_f[0][2], ctx->hs_f[0][3], ctx->hs_f[0][4], ctx->hs_pid[0],
                  ctx->hs_f[1][0], ctx->hs_f[1][1], ctx->hs_f[1][2], ctx->hs_f[1][3], ctx->hs_f[1][4], ctx->hs_pid[1],
                  closure, h_mlp, relax_w, 0, 0.f, nullptr, step, ctx->hs_mom, ctx->hs_coef, ctx->hs_flags,
                  ctx->hs_cell_start, stream);
-    if (rc != FP_OK) return rc;
-    for (int k = 0; k < 5; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(hp[k], ctx->hs_f[1][k], nb, cudaMemcpyDeviceToHost, st));
-    if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_pid, ctx->hs_pid[1], nb, cudaMemcpyDeviceToHost, st));
+    ctx->ev_before_gather = nullptr;
+    ctx->ev_after_gather = nullptr;
+    if (rc != FP_OK) { cudaStreamSynchronize(side); return rc; }
+    // device -> host: positions and ids are final after the gather and go back on the side stream while moments,
+    // closure and update run; the velocities and the per-cell outputs follow on the caller's stream
+    if (np > 0) {
+        FP_CUDA_OK(ctx, cudaStreamWaitEvent(side, ctx->hs_ev[2], 0));
+        FP_CUDA_OK(ctx, cudaMemcpyAsync(hp[0], ctx->hs_f[1][0], nb, cudaMemcpyDeviceToHost, side));
+        FP_CUDA_OK(ctx, cudaMemcpyAsync(hp[1], ctx->hs_f[1][1], nb, cudaMemcpyDeviceToHost, side));
+        FP_CUDA_OK(ctx, cudaMemcpyAsync(h_pid, ctx->hs_pid[1], nb, cudaMemcpyDeviceToHost, side));
+    }
+    for (int k = 2; k < 5; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(hp[k], ctx->hs_f[1][k], nb, cudaMemcpyDeviceToHost, st));
     if (h_coef) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_coef, ctx->hs_coef, (size_t)ctx->ncell * 9 * 4, cudaMemcpyDeviceToHost, st));
     if (h_flags) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_flags, ctx->hs_flags, (size_t)ctx->ncell * 4, cudaMemcpyDeviceToHost, st));
     if (h_cell_start) FP_CUDA_OK(ctx, cudaMemcpyAsync(h_cell_start, ctx->hs_cell_start, ((size_t)ctx->ncell + 1) * 4, cudaMemcpyDeviceToHost, st));
+    FP_CUDA_OK(ctx, cudaStreamSynchronize(side));
     FP_CUDA_OK(ctx, cudaStreamSynchronize(st));
     return FP_OK;
 }

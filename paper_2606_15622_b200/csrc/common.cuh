@@ -62,6 +62,11 @@ struct fp_ctx {
     uint32_t *hs_flags = nullptr;
     int32_t  *hs_cell_start = nullptr;
     bool      hs_ready = false;
+    // fp_step_host overlap: a side stream for the copies that need not sit on the caller's stream, and the two events
+    // the payload gather waits on / records (null outside fp_step_host)
+    cudaStream_t hs_side = nullptr;
+    cudaEvent_t  hs_ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t  ev_before_gather = nullptr, ev_after_gather = nullptr;
     fp_mlp_dev mlp;
     bool      mlp_force_fp32 = false;   // FPCL_MLP_FP32=1: always use the plain-FMA surrogate kernel
     // measurement hooks

@@ -361,6 +361,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     const int gblocks = (int)(want < cap ? want : cap);
     gather_grid Gd;
     Gd.nx = ctx->p.nx; Gd.ny = ctx->p.ny; Gd.x0 = ctx->p.x0; Gd.y0 = ctx->p.y0; Gd.inv_dx = ctx->inv_dx; Gd.inv_dy = ctx->inv_dy;
+    if (ctx->ev_before_gather) FP_CUDA_OK(ctx, cudaStreamWaitEvent(st, ctx->ev_before_gather, 0));
     if (packed)
         fp_launch(gather_kernel<true>, gblocks, 256, 0, st, np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
                   x_out, y_out, vx_out, vy_out, vz_out, pid_out, Gd);
@@ -369,6 +370,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
                   x_out, y_out, vx_out, vy_out, vz_out, pid_out, Gd);
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
+    if (ctx->ev_after_gather) FP_CUDA_OK(ctx, cudaEventRecord(ctx->ev_after_gather, st));
     if (perm) FP_CUDA_OK(ctx, cudaMemcpyAsync(perm, iin, (size_t)np * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
     return FP_OK;
 }
