@@ -345,6 +345,44 @@ def test_full_size_cavity(gpu, wl, orc):
     ctx.close()
 
 
+# ------------------------------------------------------------------------------------------------ degenerate inputs
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 700])
+@pytest.mark.parametrize("closure", [0, 1])
+def test_step_degenerate_counts(gpu, wl, orc, n, closure):
+    """No particle at all, fewer particles than the closure needs, and every particle in one cell of an otherwise
+    empty grid (one 700-particle cell: the sliced path): the whole step must agree with the oracle, flags included."""
+    import torch
+    cfg = wl.make_config(6, 5, 1.0 / 6, 0.2, 0.01, 0.8, wl.NO_WALLS, seed=77, max_particles=max(n, 1))
+    rng = np.random.default_rng(100 + n)
+    st = {"x": (2.0 / 6 + rng.uniform(0.01, 0.15, n)).astype(np.float32), "y": (0.6 + rng.uniform(0.01, 0.18, n)).astype(np.float32),
+          "vx": rng.normal(0.1, 0.7, n).astype(np.float32), "vy": rng.normal(0.0, 0.7, n).astype(np.float32),
+          "vz": rng.normal(-0.2, 0.7, n).astype(np.float32), "pid": np.arange(n, dtype=np.uint32)}
+    mlp = wl.xavier_mlp(seed=0, n_scale=1.0 / 60.0, tau=cfg["tau"], bias_scale=0.1) if closure else None
+    got, res, ref, aux = _one_step(gpu, orc, cfg, st, closure, mlp, 3)
+    assert np.array_equal(res["cell_start"], aux["cell_start"])
+    assert np.array_equal(res["flags"].view(np.uint32), aux["flags"])
+    for k in ("x", "y", "pid"):
+        assert np.array_equal(_bits(got[k]), _bits(ref[k])), k
+    occupied = aux["mom"][:, 0] > 0
+    assert np.allclose(res["mom"][:, 0], aux["mom"][:, 0])
+    if n:
+        pre = _pre(orc, st, cfg, 3)
+        r = moment_ratio(res["mom"], aux["mom"], absmom=abs_moments(pre[0], pre[1], pre[2], aux["cell_start"], aux["mom"]))
+        assert r <= 1.0, r
+        tol = 4e-6 if closure else 1e-6
+        rv = velocity_ratio((got["vx"], got["vy"], got["vz"]), (ref["vx"], ref["vy"], ref["vz"]), aux["cell_start"],
+                            _theta(aux["mom"]), tol=tol)
+        assert rv <= 1.0, rv
+    assert np.isfinite(res["coef"]).all()
+    assert (res["coef"][~occupied] == 0).all()
+
+
+def _pre(orc, st, cfg, step):
+    """cell-sorted velocities before the update (what the moments were taken of)."""
+    s2, _, _ = orc.sort_by_cell(orc.stream_walls(st, cfg, step), cfg)
+    return s2["vx"], s2["vy"], s2["vz"]
+
+
 # ------------------------------------------------------------------------------------------------ fallback paths
 def test_unstaged_paths(gpu, wl, orc):
     """Per-warp staging needs 16-byte aligned arrays and cells that fit the warp's buffer.  Unaligned views and a
