@@ -13,7 +13,7 @@
 // shared memory then holds the augmented 9x10 systems as [entry][thread] (conflict free).  Pivoting swaps rows
 // physically -- the only dynamically indexed accesses -- so the rest of the elimination is straight-line code on
 // compile-time offsets.  22.5 KB and 32 x 144 registers per warp: all 9 warps a 40k-cell grid puts on an SM are
-// resident at once.  Measured at 40k cells: elimination 8 us, assembly + back substitution 1.5 us, the rest
+// resident at once.  Measured at 40k cells (one pivot step per sweep): elimination 8 us, assembly + back substitution 1.5 us, the rest
 // (launch, staging round trip, scaling, update constants, stores) 11 us -- a latency chain, not a throughput
 // problem; a 10-lanes-per-cell cooperative solve (column per lane, shuffle broadcasts) shortened the chain but
 // executed 5x the instructions and took 44 us instead of 20.  The system never touches HBM: 232 B/cell in,
@@ -141,12 +141,16 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
         CE_ROW(0) CE_ROW(1) CE_ROW(2) CE_ROW(3) CE_ROW(4) CE_ROW(5) CE_ROW(6) CE_ROW(7) CE_ROW(8)
 #undef CE_ROW
     }
-    // ---- Gaussian elimination with partial pivoting.  Rows are swapped physically (the only dynamically indexed
-    // accesses), so every other address is a compile-time offset and the row updates of a step are independent
-    // straight-line code the scheduler can interleave -- the solve is a latency chain, not a throughput problem.
+    // ---- Gaussian elimination with partial pivoting, two pivot steps per sweep.  The sweep is shared-memory-bandwidth
+    // bound (every entry read and written once per step: ~7 KB per cell), so steps k and k+1 are fused: after pivot
+    // row k is chosen, only column k+1 is updated (in registers) to find pivot row k+1, then each remaining entry gets
+    // both updates in one read-modify-write.  Every fused multiply-add has the operands of the step-by-step
+    // algorithm, so the result is bit-identical to it.  Rows are swapped physically (the only dynamically indexed
+    // accesses); every other address is a compile-time offset.
     double minpiv = INFINITY, maxpiv = 0.0;
 #pragma unroll
-    for (int k = 0; k < 9; ++k) {
+    for (int k = 0; k < 8; k += 2) {
+        // -- pivot k
         double best = -1.0;
         int pr = k;
 #pragma unroll
@@ -157,21 +161,69 @@ closure_exact_kernel(const double* __restrict__ mom, const float* __restrict__ t
         }
         minpiv = fmin(minpiv, best);
         maxpiv = fmax(maxpiv, best);
-        double prow[10];
+        double p1[10];
 #pragma unroll
         for (int j = k; j < 10; ++j) {                // swap rows k and pr (pr == k: rewrites the same values)
-            prow[j] = CE_A(pr, j);
+            p1[j] = CE_A(pr, j);
             const double t = CE_A(k, j);
             CE_A(pr, j) = t;
-            CE_A(k, j) = prow[j];
+            CE_A(k, j) = p1[j];
         }
-        const double inv = 1.0 / prow[k];
+        const double inv1 = 1.0 / p1[k];
+        // -- multipliers of step k and column k+1 after step k, rows k+1..8, in registers
+        double f1[9], a1[9];
 #pragma unroll
         for (int r = k + 1; r < 9; ++r) {
-            const double f = CE_A(r, k) * inv;
-#pragma unroll
-            for (int j = k + 1; j < 10; ++j) CE_A(r, j) -= f * prow[j];
+            f1[r] = CE_A(r, k) * inv1;
+            a1[r] = CE_A(r, k + 1) - f1[r] * p1[k + 1];
         }
+        // -- pivot k+1 on the updated column
+        double best2 = -1.0;
+        int pr2 = k + 1;
+#pragma unroll
+        for (int r = k + 1; r < 9; ++r) {
+            double v = fabs(a1[r]);
+            if (!(v >= 0.0)) v = 0.0;
+            if (v > best2) { best2 = v; pr2 = r; }
+        }
+        minpiv = fmin(minpiv, best2);
+        maxpiv = fmax(maxpiv, best2);
+#pragma unroll
+        for (int r = k + 2; r < 9; ++r) {             // the swap of rows k+1 and pr2, register part
+            if (r == pr2) {
+                const double tf = f1[k + 1]; f1[k + 1] = f1[r]; f1[r] = tf;
+                const double ta = a1[k + 1]; a1[k + 1] = a1[r]; a1[r] = ta;
+            }
+        }
+        // -- pivot row k+1 after step k; the not yet updated row that was at k+1 moves to pr2
+        double p2[10];
+        p2[k + 1] = a1[k + 1];
+#pragma unroll
+        for (int j = k + 2; j < 10; ++j) {
+            const double u = CE_A(pr2, j);
+            const double t = CE_A(k + 1, j);
+            CE_A(pr2, j) = t;
+            p2[j] = u - f1[k + 1] * p1[j];
+        }
+#pragma unroll
+        for (int j = k + 1; j < 10; ++j) CE_A(k + 1, j) = p2[j];
+        const double inv2 = 1.0 / p2[k + 1];
+        // -- both updates of the remaining rows in one pass
+#pragma unroll
+        for (int r = k + 2; r < 9; ++r) {
+            const double f2 = a1[r] * inv2;
+#pragma unroll
+            for (int j = k + 2; j < 10; ++j) {
+                const double t = CE_A(r, j) - f1[r] * p1[j];
+                CE_A(r, j) = t - f2 * p2[j];
+            }
+        }
+    }
+    {   // the last pivot (k = 8): nothing left to eliminate
+        double v = fabs(CE_A(8, 8));
+        if (!(v >= 0.0)) v = 0.0;
+        minpiv = fmin(minpiv, v);
+        maxpiv = fmax(maxpiv, v);
     }
     // ---- back substitution
     double y[9];
