@@ -29,9 +29,11 @@
 
 // One cell per group of G lanes.  bx/by/bz: the warp's private staging copy in shared memory, particle p at b?[p];
 // pass 1 overwrites v by v - v_pivot.
-template <int G, bool FULL>
+struct mom_no_hook { __device__ __forceinline__ void operator()() const {} };
+
+template <int G, bool FULL, class Hook = mom_no_hook>
 __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,
-                                               bool have, int gl, double* __restrict__ rec)
+                                               bool have, int gl, double* __restrict__ rec, Hook after_reads = Hook())
 {
     float* wx = const_cast<float*>(bx);
     float* wy = const_cast<float*>(by);
@@ -119,6 +121,7 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
                 Gm[0] = fpd_fma2(c2, cx, Gm[0]); Gm[1] = fpd_fma2(c2, cy, Gm[1]); Gm[2] = fpd_fma2(c2, cz, Gm[2]);   // h_i
             }
         }
+        if (c0 + G * MOM_CHUNK_PER_LANE >= nmax) after_reads();     // the staging buffer is not read again
         const float P0 = P[0].x + P[0].y, P1 = P[1].x + P[1].y, P2 = P[2].x + P[2].y, P3 = P[3].x + P[3].y,
                     P4 = P[4].x + P[4].y, P5 = P[5].x + P[5].y;
         const float t0 = T[0].x + T[0].y, t1 = T[1].x + T[1].y, t2 = T[2].x + T[2].y, t3 = T[3].x + T[3].y,
@@ -155,6 +158,149 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
             else if (slot == 1) val = n > 0 ? (double)px + m0d : 0.0;
             else if (slot == 2) val = n > 0 ? (double)py + m1d : 0.0;
             else if (slot == 3) val = n > 0 ? (double)pz + m2d : 0.0;
+            if (slot < NREC) rec[slot] = val;
+        }
+    }
+}
+
+// The common case, cells of at most 128*G particles: same two passes, but (i) the particles of a cell are visited in
+// rotated order, starting at the particle whose shared-memory bank is G*group, so that the 32 lanes of a warp hit 32
+// different banks in every load whatever the cell boundaries are (the lanes of a group step through the cell
+// 2G particles at a time; only the part after the wrap-around can conflict); (ii) nothing is parked: pass 2 forms
+// (v - v_pivot) - m again; (iii) per-lane sums stay fp32 for the whole cell (<= 64 terms per packed half, as in the
+// chunked path) and go straight to the cross-lane tree.  `after_reads` runs once the staging buffer is not needed
+// any more.  Lanes of different groups run different trip counts; the (masked) last step is peeled.
+template <int G, bool FULL, class Hook>
+__device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,
+                                             bool have, int gl, int group, double* __restrict__ rec, Hook after_reads)
+{
+    constexpr int NP = (FULL || G > 16) ? 32 : 16;
+    constexpr int NREC = FULL ? 29 : 13;
+    constexpr int PER = NP / G;
+    const float* x = bx + s;
+    const float* y = by + s;
+    const float* z = bz + s;
+    float px = 0.f, py = 0.f, pz = 0.f;
+    if (n > 0) { px = x[0]; py = y[0]; pz = z[0]; }
+    const float2 npx = fpd_dup(-px), npy = fpd_dup(-py), npz = fpd_dup(-pz);
+    // rotation: particle o of the cell sits in bank G*group
+    int32_t o = (int32_t)((uint32_t)(G * group) - (fpt_smem_u32(x) >> 2)) & 31;
+    while (n > 0 && o >= n) o -= n;
+    if (n <= 0) o = 0;
+    const int32_t full = n / (2 * G);                       // steps in which all 2G particles exist
+    const int32_t t0 = 2 * G * full + gl, t1 = t0 + G;      // the peeled last step
+    const bool v0 = t0 < n, v1 = t1 < n;
+    int32_t q0 = o + t0, q1 = o + t1;
+    if (q0 >= n) q0 -= n;
+    if (q1 >= n) q1 -= n;
+    if (!v0) q0 = 0;
+    if (!v1) q1 = 0;
+    const float2 msk = make_float2(v0 ? 1.f : 0.f, v1 ? 1.f : 0.f);
+    int32_t j0s = o + gl, j1s = o + gl + G;
+    if (j0s >= n) j0s -= n;
+    if (j1s >= n) j1s -= n;
+    // ---- pass 1: mean about the pivot
+    float2 A0 = fpd_dup(0.f), A1 = fpd_dup(0.f), A2 = fpd_dup(0.f);
+    {
+        int32_t j0 = j0s, j1 = j1s;
+#pragma unroll 2
+        for (int32_t k = 0; k < full; ++k) {
+            A0 = fpd_add2(A0, fpd_add2(make_float2(x[j0], x[j1]), npx));
+            A1 = fpd_add2(A1, fpd_add2(make_float2(y[j0], y[j1]), npy));
+            A2 = fpd_add2(A2, fpd_add2(make_float2(z[j0], z[j1]), npz));
+            j0 += 2 * G; j1 += 2 * G;
+            if (j0 >= n) j0 -= n;
+            if (j1 >= n) j1 -= n;
+        }
+        A0 = fpd_fma2(fpd_add2(make_float2(x[q0], x[q1]), npx), msk, A0);
+        A1 = fpd_fma2(fpd_add2(make_float2(y[q0], y[q1]), npy), msk, A1);
+        A2 = fpd_fma2(fpd_add2(make_float2(z[q0], z[q1]), npz), msk, A2);
+    }
+    double S0 = (double)A0.x + (double)A0.y, S1 = (double)A1.x + (double)A1.y, S2 = (double)A2.x + (double)A2.y;
+#pragma unroll
+    for (int d = G / 2; d >= 1; d >>= 1) {
+        S0 += fpd_shfl_xor(S0, d); S1 += fpd_shfl_xor(S1, d); S2 += fpd_shfl_xor(S2, d);
+    }
+    const double invn = n > 0 ? 1.0 / (double)n : 0.0;
+    const double m0d = S0 * invn, m1d = S1 * invn, m2d = S2 * invn;
+    const float2 nm0 = fpd_dup(-(float)m0d), nm1 = fpd_dup(-(float)m1d), nm2 = fpd_dup(-(float)m2d);
+    // ---- pass 2: central moments
+    float2 P[6], T[10], F[6], Gm[3];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { P[k] = fpd_dup(0.f); F[k] = fpd_dup(0.f); }
+#pragma unroll
+    for (int k = 0; k < 10; ++k) T[k] = fpd_dup(0.f);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) Gm[k] = fpd_dup(0.f);
+    auto accumulate = [&](const float2 cx, const float2 cy, const float2 cz) {
+        const float2 xx = fpd_mul2(cx, cx), xy = fpd_mul2(cx, cy), xz = fpd_mul2(cx, cz);
+        const float2 yy = fpd_mul2(cy, cy), yz = fpd_mul2(cy, cz), zz = fpd_mul2(cz, cz);
+        const float2 c2 = fpd_add2(fpd_add2(xx, yy), zz);
+        P[0] = fpd_add2(P[0], xx); P[1] = fpd_add2(P[1], xy); P[2] = fpd_add2(P[2], xz);
+        P[3] = fpd_add2(P[3], yy); P[4] = fpd_add2(P[4], yz); P[5] = fpd_add2(P[5], zz);
+        if (FULL) {
+            T[0] = fpd_fma2(xx, cx, T[0]); T[1] = fpd_fma2(xx, cy, T[1]); T[2] = fpd_fma2(xx, cz, T[2]);
+            T[3] = fpd_fma2(xy, cy, T[3]); T[4] = fpd_fma2(xy, cz, T[4]); T[5] = fpd_fma2(xz, cz, T[5]);
+            T[6] = fpd_fma2(yy, cy, T[6]); T[7] = fpd_fma2(yy, cz, T[7]); T[8] = fpd_fma2(yz, cz, T[8]);
+            T[9] = fpd_fma2(zz, cz, T[9]);
+            F[0] = fpd_fma2(c2, xx, F[0]); F[1] = fpd_fma2(c2, xy, F[1]); F[2] = fpd_fma2(c2, xz, F[2]);
+            F[3] = fpd_fma2(c2, yy, F[3]); F[4] = fpd_fma2(c2, yz, F[4]); F[5] = fpd_fma2(c2, zz, F[5]);
+            const float2 c4 = fpd_mul2(c2, c2);
+            Gm[0] = fpd_fma2(c4, cx, Gm[0]); Gm[1] = fpd_fma2(c4, cy, Gm[1]); Gm[2] = fpd_fma2(c4, cz, Gm[2]);
+        } else {
+            Gm[0] = fpd_fma2(c2, cx, Gm[0]); Gm[1] = fpd_fma2(c2, cy, Gm[1]); Gm[2] = fpd_fma2(c2, cz, Gm[2]);   // h_i
+        }
+    };
+    {
+        int32_t j0 = j0s, j1 = j1s;
+#pragma unroll 1
+        for (int32_t k = 0; k < full; ++k) {
+            const float2 cx = fpd_add2(fpd_add2(make_float2(x[j0], x[j1]), npx), nm0);
+            const float2 cy = fpd_add2(fpd_add2(make_float2(y[j0], y[j1]), npy), nm1);
+            const float2 cz = fpd_add2(fpd_add2(make_float2(z[j0], z[j1]), npz), nm2);
+            j0 += 2 * G; j1 += 2 * G;
+            if (j0 >= n) j0 -= n;
+            if (j1 >= n) j1 -= n;
+            accumulate(cx, cy, cz);
+        }
+        const float2 cx = fpd_mul2(fpd_add2(fpd_add2(make_float2(x[q0], x[q1]), npx), nm0), msk);
+        const float2 cy = fpd_mul2(fpd_add2(fpd_add2(make_float2(y[q0], y[q1]), npy), nm1), msk);
+        const float2 cz = fpd_mul2(fpd_add2(fpd_add2(make_float2(z[q0], z[q1]), npz), nm2), msk);
+        accumulate(cx, cy, cz);
+    }
+    after_reads();                                           // the staging buffer is not read again
+    float r[NP];
+    r[0] = r[1] = r[2] = r[3] = 0.f;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) r[4 + k] = P[k].x + P[k].y;
+    if (FULL) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) r[10 + k] = T[k].x + T[k].y;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) r[20 + k] = F[k].x + F[k].y;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) r[26 + k] = Gm[k].x + Gm[k].y;
+#pragma unroll
+        for (int k = 29; k < NP; ++k) r[k] = 0.f;
+    } else {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) r[10 + k] = Gm[k].x + Gm[k].y;
+#pragma unroll
+        for (int k = 13; k < NP; ++k) r[k] = 0.f;
+    }
+    fpd_transpose_reduce<NP, G, float>(r, gl);           // balanced fp32 tree over the group's partial sums
+    // lane gl holds record slots PER*gl .. PER*gl + PER - 1
+    if (have) {
+#pragma unroll
+        for (int i = 0; i < PER; ++i) {
+            const int slot = PER * gl + i;
+            double val = (double)r[i] * invn;
+            if (i < 4) {                                     // slots 0..3 (N, U) can only sit at i < 4
+                if (slot == 0) val = (double)n;
+                else if (slot == 1) val = n > 0 ? (double)px + m0d : 0.0;
+                else if (slot == 2) val = n > 0 ? (double)py + m1d : 0.0;
+                else if (slot == 3) val = n > 0 ? (double)pz + m2d : 0.0;
+            }
             if (slot < NREC) rec[slot] = val;
         }
     }
@@ -269,11 +415,26 @@ __device__ __noinline__ void mom_dense_chunk(const float* __restrict__ vx, const
     }
 }
 
-// Persistent warps: a warp owns chunks wg, wg + nwarps, ... of 32/G consecutive cells; while it reduces one chunk the
-// bulk copies of its next chunk are already in flight into the warp's other staging buffer (2-stage pipeline per
-// warp, mbarrier per stage), and the cell boundaries of the chunk after that are being fetched.
+// Persistent warps: a warp owns chunks wg, wg + nwarps, ... of 32/G consecutive cells.  MOM_STAGES = 2: while it reduces
+// one chunk the bulk copies of its next chunk are already in flight into the warp's other staging buffer (mbarrier
+// per stage).  MOM_STAGES = 1: one (larger) buffer per warp; the copies of the next chunk are issued as soon as pass 2
+// has read the last particle, i.e. they overlap the cross-lane tree, the fp64 finish and the record stores, and the
+// other resident warps cover the rest of the latency.  The cell boundaries of the chunk after next are fetched ahead
+// in both cases.
 #ifndef MOM_MINB
 #define MOM_MINB 4                      // 128 registers: four CTAs per SM is what the staging buffers allow
+#endif
+#ifndef MOM_STAGES
+#define MOM_STAGES 2
+#endif
+#ifndef MOM_ROT
+#define MOM_ROT 1                       // rotated, conflict-free visiting order for cells of <= 128*G particles
+#endif
+#ifndef MOM_GMIN
+#define MOM_GMIN 4                      // smallest group width instantiated for the dispatch
+#endif
+#ifndef MOM_FILL
+#define MOM_FILL 0.875                  // a chunk of 32/G mean-sized cells fills at most this part of the buffer
 #endif
 template <int G, bool FULL>
 __global__ void __launch_bounds__(MOM_THREADS, MOM_MINB)
@@ -284,16 +445,17 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
     fpd_pdl();
     constexpr int NREC = FULL ? 29 : 13;
     constexpr int CPW = 32 / G;                          // cells per warp and chunk
+    constexpr int NST = MOM_STAGES;
     extern __shared__ __align__(16) unsigned char fpw_smem[];
-    float* stage = reinterpret_cast<float*>(fpw_smem);                                   // [MOM_WARPS][2][3][MOM_CAP]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(fpw_smem + (size_t)MOM_WARPS * 6 * MOM_CAP * sizeof(float));
+    float* stage = reinterpret_cast<float*>(fpw_smem);                                   // [MOM_WARPS][NST][3][MOM_CAP]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(fpw_smem + (size_t)MOM_WARPS * NST * 3 * MOM_CAP * sizeof(float));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gl = lane & (G - 1), group = lane / G;
     const int64_t nchunks = ((int64_t)ncell + CPW - 1) / CPW;
     const int64_t nw = (int64_t)gridDim.x * MOM_WARPS;
     int64_t chunk = (int64_t)blockIdx.x * MOM_WARPS + warp;
     if (chunk >= nchunks) return;
-    float* wbuf = stage + (size_t)warp * 6 * MOM_CAP;
+    float* wbuf = stage + (size_t)warp * NST * 3 * MOM_CAP;
     uint64_t* wbar = bars + warp * 2;
     if (lane == 0) { fpt_mbar_init(&wbar[0], 1); fpt_mbar_init(&wbar[1], 1); }
     __syncwarp();
@@ -320,10 +482,13 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
     uint32_t phase = 0;
     while (true) {
         fpw_range r_nxt = r_cur;
-        if (nxt < nchunks) {
+        const bool more = nxt < nchunks;
+        if (more) {
             r_nxt = range_of(cs_nxt);
-            __syncwarp();                                   // every lane is done reading buffer b^1 (previous chunk)
-            issue(r_nxt, b ^ 1);
+            if (NST == 2) {
+                __syncwarp();                               // every lane is done reading buffer b^1 (previous chunk)
+                issue(r_nxt, b ^ 1);
+            }
         }
         const int64_t nxt2 = nxt + nw;
         const int32_t cs_nxt2 = nxt2 < nchunks ? load_cs(nxt2) : 0;
@@ -333,6 +498,7 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
         const bool have = cell < ncell;
         const int32_t n = have ? e - s : 0;
         double* rec = mom + (size_t)(have ? cell : 0) * NREC;
+        bool reissued = false;
         if (r_cur.staged) {
             float* sx = wbuf + (size_t)b * 3 * MOM_CAP;
             float* sy = sx + MOM_CAP;
@@ -343,16 +509,45 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
             }
             if (r_cur.nb > 0) { fpt_mbar_wait(&wbar[b], (phase >> b) & 1u); phase ^= 1u << b; }
             __syncwarp();
-            mom_cell_group<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, s, n, have, gl, rec);   // shared-memory loads
+            const int32_t nmax = __reduce_max_sync(0xffffffffu, n);
+            const int32_t sb = n > 0 ? s : r_cur.a0;        // empty cell: any staged address
+            if (MOM_ROT && nmax <= 128 * G) {
+                auto hook = [&]() {
+                    if (NST == 1 && more) {
+                        fpt_fence_proxy_async();
+                        __syncwarp();
+                        issue(r_nxt, 0);
+                    }
+                    reissued = true;
+                };
+                mom_cell_rot<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, sb, n, have, gl, group, rec, hook);
+            } else if (NST == 1) {
+                auto hook = [&]() {
+                    if (more) {
+                        fpt_fence_proxy_async();            // generic-proxy writes of pass 1 vs the new bulk copy
+                        __syncwarp();
+                        issue(r_nxt, 0);
+                    }
+                    reissued = true;
+                };
+                mom_cell_group<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, s, n, have, gl, rec, hook);
+            } else {
+                mom_cell_group<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, s, n, have, gl, rec);
+            }
         } else {
             // a chunk too dense for the staging buffer (load-imbalanced grids): cell by cell in buffer b
             mom_dense_chunk<FULL>(vx, vy, vz, cs_cur, CPW, chunk, ncell, np, aligned, wbuf + (size_t)b * 3 * MOM_CAP,
                                   &wbar[b], phase, b, lane, mom);
         }
-        if (nxt >= nchunks) break;
+        if (!more) break;
+        if (NST == 1 && !reissued) {
+            fpt_fence_proxy_async();
+            __syncwarp();
+            issue(r_nxt, 0);
+        }
         chunk = nxt; cs_cur = cs_nxt; r_cur = r_nxt;
         nxt = nxt2; cs_nxt = cs_nxt2;
-        b ^= 1;
+        if (NST == 2) b ^= 1;
     }
 }
 
@@ -362,7 +557,7 @@ static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float
 {
     const int cells_per_block = MOM_WARPS * (32 / G);
     const int aligned = ((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0 ? 1 : 0;
-    const size_t smem = (size_t)MOM_WARPS * 6 * MOM_CAP * sizeof(float) + MOM_WARPS * 2 * sizeof(uint64_t);
+    const size_t smem = (size_t)MOM_WARPS * MOM_STAGES * 3 * MOM_CAP * sizeof(float) + MOM_WARPS * 2 * sizeof(uint64_t);
     static int occ = 0;                           // resident CTAs per SM, one value per instantiation (G)
     if (occ == 0) {
         cudaFuncSetAttribute(moments_warp_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -386,10 +581,17 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     cudaStream_t st = (cudaStream_t)stream;
     const double ppc = (double)np / (double)ctx->ncell;
     // group width: the chunk of 32/G cells must fit the staging buffer (tiles.cuh)
-    if (ppc >= FPW_G32_MIN)      launch_moments<32>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    else if (ppc >= FPW_G16_MIN) launch_moments<16>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    else if (ppc >= FPW_G8_MIN)  launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
-    else                   launch_moments<4>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    // lanes per cell: the smallest G whose chunk of 32/G mean-sized cells leaves room for the count fluctuations
+    const double room = MOM_FILL * (double)MOM_CAP;
+    if (ppc * 2 > room)                        launch_moments<32>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else if (ppc * 4 > room)                   launch_moments<16>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else if (ppc * 8 > room)                   launch_moments<8>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+#if MOM_GMIN <= 2
+    else if (ppc * 16 > room)                  launch_moments<4>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+    else                                       launch_moments<2>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+#else
+    else                                       launch_moments<4>(ctx, np, vx, vy, vz, cell_start, mode, mom, st);
+#endif
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);
     return FP_OK;
