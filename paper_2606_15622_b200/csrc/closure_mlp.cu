@@ -33,6 +33,7 @@ struct mlp_src {
 static inline int pad8(int v) { return (v + 7) & ~7; }
 
 #include "mlp_tc.cuh"
+#include "mlp_wide.cuh"
 
 // repack caller weights [out][in] -> blob Wt[in][out_pad], bias[out_pad] (zero padded), scalers appended
 __global__ void mlp_pack_kernel(const __grid_constant__ mlp_desc D, const __grid_constant__ mlp_src S,
@@ -250,6 +251,40 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         const int want = fp_div_up(fp_div_up(ctx->ncell, 16), TC_WARPS);
         const int cap = ctx->num_sms * occ;
         fp_launch(mlp_tc_kernel, want < cap ? want : cap, TC_THREADS, smem, st, mom, tau_cell, frags, misc, coef, flags, P);
+        FP_LAUNCH_OK(ctx);
+        FP_COUNT(ctx, 2);
+        return FP_OK;
+    }
+    // ---- tensor-core path for wide networks [13|16]-256-...-256-9 (the paper's own shape, mlp_wide.cuh)
+    bool wide = !ctx->mlp_force_fp32 && M.n_layers >= 2;
+    for (int l = 1; l < M.n_layers && wide; ++l) wide = D.dims[l] == WD_H;
+    if (wide) {
+        const size_t fbytes = wd_frag_total(M.n_layers) * sizeof(uint4);
+        const size_t mbytes = (size_t)wd_misc_floats(M.n_layers) * sizeof(float);
+        if (C.wd_bytes < fbytes + mbytes) {
+            if (C.wd_frags) FP_CUDA_OK(ctx, cudaFree(C.wd_frags));
+            C.wd_frags = nullptr; C.wd_bytes = 0;
+            FP_CUDA_OK(ctx, cudaMalloc((void**)&C.wd_frags, fbytes + mbytes));
+            C.wd_bytes = fbytes + mbytes;
+        }
+        uint4* frags = reinterpret_cast<uint4*>(C.wd_frags);
+        float* misc = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(C.wd_frags) + fbytes);
+        fp_launch(mlpw_pack_kernel, 2 * ctx->num_sms, 256, 0, st, S, M.n_layers, D.dims[0], frags, misc);
+        wd_params P;
+        P.stride = mom_stride; P.feature_set = M.feature_set; P.act = M.act; P.min_count = ctx->p.min_count_mlp;
+        P.ncell = ctx->ncell; P.nin = D.dims[0]; P.n_layers = M.n_layers; P.tau_scalar = ctx->p.tau;
+        P.n_scale = M.n_scale; P.theta_ref = M.theta_ref; P.relax_w = relax_w;
+        P.dt = ctx->p.dt; P.eps2_scale = ctx->p.eps2_scale; P.cellc = cellc;
+        const size_t smem = (size_t)4 * WD_M * WD_XS * sizeof(__nv_bfloat16) +
+                            (size_t)((wd_misc_floats(M.n_layers) + 3) & ~3) * sizeof(float) + (size_t)WD_M * 17 * sizeof(float);
+        static bool attr_set = false;
+        if (!attr_set) {
+            FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            attr_set = true;
+        }
+        const int want = fp_div_up(ctx->ncell, WD_M);
+        fp_launch(mlp_wide_kernel, want < ctx->num_sms ? want : ctx->num_sms, WD_THREADS, smem, st, mom, tau_cell,
+                  (const uint4*)frags, (const float*)misc, coef, flags, P);
         FP_LAUNCH_OK(ctx);
         FP_COUNT(ctx, 2);
         return FP_OK;

@@ -28,6 +28,8 @@ struct fp_mlp_dev {                 // uploaded copy of the caller's MLP (fp_clo
     int32_t  act = 0, feature_set = 0;
     float    n_scale = 1.f, theta_ref = 0.5f;
     float*   tc_frags = nullptr;    // device: packed 3xTF32 mma fragments + biases/scalers (mlp_tc.cuh)
+    float*   wd_frags = nullptr;    // device: packed split-bf16 mma fragments + biases/scalers (mlp_wide.cuh)
+    size_t   wd_bytes = 0;
     float*   blob = nullptr;        // device: [W0 | b0 | W1 | b1 | ... | x_mean | x_scale | y_mean | y_scale]
     size_t   blob_floats = 0;
     size_t   w_off[FPCL_MAX_LAYERS] = {0}, b_off[FPCL_MAX_LAYERS] = {0};
