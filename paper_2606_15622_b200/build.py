@@ -30,7 +30,8 @@ def _newer(target, deps):
 
 def build(force=False, verbose=False):
     os.makedirs(OBJDIR, exist_ok=True)
-    headers = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "tiles.cuh"), os.path.join(INCLUDE, "fpcl.h"), os.path.abspath(__file__)]
+    headers = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")) + [
+        os.path.join(INCLUDE, "fpcl.h"), os.path.abspath(__file__)]
     jobs = []
     objs = []
     for s in SOURCES:

@@ -12,11 +12,10 @@
 //   bf16 (or TF32) product is outside north_star's 3e-3 on a four-layer network (mlp_tc.cuh measured 7e-3 for
 //   TF32 on three layers); the split form measures ~1e-5 of the output scale.
 //   layouts: activations are split once, when a layer's epilogue writes them, and stored as two bf16 arrays
-//   xh/xl[64][H + 16] (row stride = 32 mod 128 bytes: the 8-byte A-fragment loads are conflict free).  The K index
-//   of a layer is a summation index and may be permuted: k-slots (2t, 2t+1, 2t+8, 2t+9) of k-step j carry inputs
-//   16j + 4t .. 16j + 4t + 3, so a lane's A fragment is one 8-byte load per row and part; the weights are packed
-//   in the matching order, already split, one uint4 {b0_hi, b1_hi, b0_lo, b1_lo} per (layer, k-step, n-tile, lane),
-//   by mlpw_pack_kernel.
+//   xh/xl[64][H + 8] (row stride = 16 mod 128 bytes: ldmatrix.x4 rows and the epilogue's 4-byte stores are both
+//   conflict free); one ldmatrix.x4 per m-tile, k-step and part delivers the A fragment as an aligned register
+//   quad.  The weights are packed in fragment order, already split, one uint4 {b0_hi, b1_hi, b0_lo, b1_lo} per
+//   (layer, k-step, n-tile, lane), by mlpw_pack_kernel.
 // Features, standardisation, fallback policy, under-relaxation and the update constants are those of the fp32
 // kernel (closure_mlp.cu).
 #pragma once
@@ -54,13 +53,13 @@ __device__ __forceinline__ void wd_split2(float x0, float x1, uint32_t& hi, uint
 }
 __device__ __forceinline__ void wd_mma(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
 {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
 // Pack caller weights W[l] ([out][in] row-major) into split bf16 mma B fragments.  Fragment (l, j, n, lane):
-// g = lane / 4, t = lane % 4, out = 8 n + g, in = 16 j + 4 t + q (q = 0..3): b0 = (q 0, 1), b1 = (q 2, 3).
+// g = lane / 4, t = lane % 4, out = 8 n + g: b0 = inputs (16 j + 2 t, + 1), b1 = inputs (16 j + 2 t + 8, + 9).
 __global__ void mlpw_pack_kernel(const __grid_constant__ mlp_src S, int32_t n_layers, int32_t nin,
                                  uint4* __restrict__ frags, float* __restrict__ misc)
 {
@@ -81,10 +80,13 @@ __global__ void mlpw_pack_kernel(const __grid_constant__ mlp_src S, int32_t n_la
         const int ni = (l == 0) ? nin : WD_H, no = (l == n_layers - 1) ? 9 : WD_H;
         const int lane = (int)(r & 31), n = (int)((r >> 5) % NT), j = (int)((r >> 5) / NT);
         const int g = lane >> 2, t = lane & 3;
-        const int o = 8 * n + g, i0 = 16 * j + 4 * t;
+        const int o = 8 * n + g, i0 = 16 * j + 2 * t;
         float w[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) w[q] = (o < no && i0 + q < ni) ? S.W[l][(size_t)o * ni + i0 + q] : 0.0f;
+        for (int q = 0; q < 4; ++q) {
+            const int i = i0 + (q & 1) + 8 * (q >> 1);
+            w[q] = (o < no && i < ni) ? S.W[l][(size_t)o * ni + i] : 0.0f;
+        }
         uint4 f;
         wd_split2(w[0], w[1], f.x, f.z);
         wd_split2(w[2], w[3], f.y, f.w);
@@ -106,7 +108,17 @@ __global__ void mlpw_pack_kernel(const __grid_constant__ mlp_src S, int32_t n_la
     }
 }
 
-#define WD_XS (WD_H + 16)                         // activation row stride in bf16 elements (544 bytes)
+#define WD_XS (WD_H + 8)                          // activation row stride in bf16 elements (528 bytes)
+
+// A fragment (16 cells x 16 inputs) of the m-tile starting at row r0, k-step j: lane i supplies the address of row
+// r0 + (i & 7) + 8 * ((i >> 3) & 1), inputs 16 j + 8 * (i >> 4)
+__device__ __forceinline__ void wd_ldmatrix(uint32_t (&a)[4], const __nv_bfloat16* x, int r0, int j, int lane)
+{
+    const __nv_bfloat16* p = x + (size_t)(r0 + (lane & 7) + 8 * ((lane >> 3) & 1)) * WD_XS + 16 * j + 8 * (lane >> 4);
+    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(p);
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3]) : "r"(addr) : "memory");
+}
 
 // One dense layer of width H on the CTA's 64-cell tile: warp (wm, wn) computes cells 32 wm .. +31, units 64 wn ..
 // +63 (2 m-tiles x 8 n-tiles), KS k-steps of 16 inputs; bias, activation, split and store into the other buffer.
@@ -126,41 +138,42 @@ __device__ __forceinline__ void wd_layer(const __nv_bfloat16* __restrict__ xh, c
         for (int mt = 0; mt < 2; ++mt) { acc[mt][n][0] = b0; acc[mt][n][1] = b1; acc[mt][n][2] = b0; acc[mt][n][3] = b1; }
     }
     const uint4* wp = wf + (size_t)(8 * wn) * 32 + lane;                 // + (j * NT + n) * 32
-    uint4 wb[8];
-#pragma unroll
-    for (int n = 0; n < 8; ++n) wb[n] = __ldg(wp + (size_t)n * 32);
     const int row0 = 32 * wm + g;
-#pragma unroll 2
-    for (int j = 0; j < KS; ++j) {
-        uint4 wnx[8];
-        if (j + 1 < KS) {
+    auto load_w = [&](uint4 (&w)[8], int j) {
 #pragma unroll
-            for (int n = 0; n < 8; ++n) wnx[n] = __ldg(wp + ((size_t)(j + 1) * NT + n) * 32);
-        }
+        for (int n = 0; n < 8; ++n) w[n] = __ldg(wp + ((size_t)j * NT + n) * 32);
+    };
+    auto kstep = [&](const uint4 (&w)[8], int j) {
         uint32_t ahi[2][4], alo[2][4];
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt) {
-            const int r = row0 + 16 * mt;
-            const uint2 h0 = *reinterpret_cast<const uint2*>(xh + (size_t)r * WD_XS + 16 * j + 4 * t);
-            const uint2 h1 = *reinterpret_cast<const uint2*>(xh + (size_t)(r + 8) * WD_XS + 16 * j + 4 * t);
-            const uint2 l0 = *reinterpret_cast<const uint2*>(xl + (size_t)r * WD_XS + 16 * j + 4 * t);
-            const uint2 l1 = *reinterpret_cast<const uint2*>(xl + (size_t)(r + 8) * WD_XS + 16 * j + 4 * t);
-            ahi[mt][0] = h0.x; ahi[mt][1] = h1.x; ahi[mt][2] = h0.y; ahi[mt][3] = h1.y;
-            alo[mt][0] = l0.x; alo[mt][1] = l1.x; alo[mt][2] = l0.y; alo[mt][3] = l1.y;
+            wd_ldmatrix(ahi[mt], xh, 32 * wm + 16 * mt, j, lane);
+            wd_ldmatrix(alo[mt], xl, 32 * wm + 16 * mt, j, lane);
         }
+        // three sweeps over the 16 independent accumulator tiles (small terms first), so that consecutive mma
+        // instructions never depend on one another
 #pragma unroll
-        for (int n = 0; n < 8; ++n) {
+        for (int n = 0; n < 8; ++n)
 #pragma unroll
-            for (int mt = 0; mt < 2; ++mt) {
-                wd_mma(acc[mt][n], alo[mt], wb[n].x, wb[n].y);           // small terms first
-                wd_mma(acc[mt][n], ahi[mt], wb[n].z, wb[n].w);
-                wd_mma(acc[mt][n], ahi[mt], wb[n].x, wb[n].y);
-            }
-        }
-        if (j + 1 < KS) {
+            for (int mt = 0; mt < 2; ++mt) wd_mma(acc[mt][n], alo[mt], w[n].x, w[n].y);
 #pragma unroll
-            for (int n = 0; n < 8; ++n) wb[n] = wnx[n];
-        }
+        for (int n = 0; n < 8; ++n)
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) wd_mma(acc[mt][n], ahi[mt], w[n].z, w[n].w);
+#pragma unroll
+        for (int n = 0; n < 8; ++n)
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) wd_mma(acc[mt][n], ahi[mt], w[n].x, w[n].y);
+    };
+    // weights of the next k-step are in flight while this one is multiplied: two register buffers, no copies
+    uint4 w0[8], w1[8];
+    load_w(w0, 0);
+#pragma unroll
+    for (int j = 0; j < KS; j += 2) {
+        if (j + 1 < KS) load_w(w1, j + 1);
+        kstep(w0, j);
+        if (j + 2 < KS) load_w(w0, j + 2);
+        if (j + 1 < KS) kstep(w1, j + 1);
     }
     // epilogue: activation, split, store (c0, c1) -> row g, (c2, c3) -> row g + 8, columns 8n + 2t, +1
 #pragma unroll
@@ -287,11 +300,9 @@ mlp_wide_kernel(const double* __restrict__ mom, const float* __restrict__ tau_ce
 #pragma unroll 4
             for (int j = 0; j < WD_H / 16; ++j) {
                 const uint4 w = __ldg(f_head + ((size_t)j * 2 + nt) * 32 + lane);
-                const uint2 h0 = *reinterpret_cast<const uint2*>(xh + (size_t)r * WD_XS + 16 * j + 4 * t);
-                const uint2 h1 = *reinterpret_cast<const uint2*>(xh + (size_t)(r + 8) * WD_XS + 16 * j + 4 * t);
-                const uint2 l0 = *reinterpret_cast<const uint2*>(xl + (size_t)r * WD_XS + 16 * j + 4 * t);
-                const uint2 l1 = *reinterpret_cast<const uint2*>(xl + (size_t)(r + 8) * WD_XS + 16 * j + 4 * t);
-                const uint32_t ahi[4] = {h0.x, h1.x, h0.y, h1.y}, alo[4] = {l0.x, l1.x, l0.y, l1.y};
+                uint32_t ahi[4], alo[4];
+                wd_ldmatrix(ahi, xh, 16 * mt, j, lane);
+                wd_ldmatrix(alo, xl, 16 * mt, j, lane);
                 wd_mma(c, alo, w.x, w.y);
                 wd_mma(c, ahi, w.z, w.w);
                 wd_mma(c, ahi, w.x, w.y);
