@@ -289,6 +289,57 @@ def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
     return res
 
 
+def paper_surrogate(fpcl, torch, workloads, tau):
+    """the paper's own surrogate (16 features -> 4 x 256 ReLU -> 9) with
+    under-relaxation w = 0.2 (:568), on LITE records of C3-sized (40k cells) and C5-sized (120k cells) grids.
+    Tensor-core kernel (mlp_wide.cuh): split-bf16 products, three mma per useful product."""
+    bf16_peak, src = 2250.0, "nominal dense bf16 (B200_PROFILING.md)"
+    try:
+        bf16_peak, src = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["bf16_tflops"]), "measured cuBLAS bf16 (MEASURED_PEAKS.json)"
+    except Exception:
+        pass
+    dims = (16, 256, 256, 256, 256, 9)
+    mac = sum(dims[i] * dims[i + 1] for i in range(len(dims) - 1))
+    res = {"network": "16-256-256-256-256-9 ReLU, %d parameters, relax_w = 0.2" % (mac + sum(dims[1:])),
+           "kernel": "mma.sync m16n8k16 bf16, 3 split products per useful product (~2.5e-5 of the output scale vs the oracle)",
+           "peak_source": src}
+    mlp = fpcl.Mlp(workloads.xavier_mlp(dims=dims, seed=0, act=1, feature_set=1, n_scale=0.05, tau=tau))
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
+    for name, n in (("cells_40000", 200), ("cells_119716", 346)):
+        cfg, _ = workloads.cavity(n=n, ppc=30, kn=0.5, seed=3, shuffle=False)
+        ctx = fpcl.Context(cfg)
+        ncell = ctx.ncell
+        g = torch.Generator(device="cuda"); g.manual_seed(11)
+        cnt = torch.poisson(torch.full((ncell,), 20.0, device="cuda"), generator=g).to(torch.int32)
+        cs = torch.zeros(ncell + 1, dtype=torch.int32, device="cuda"); cs[1:] = torch.cumsum(cnt, 0)
+        npart = int(cs[-1])
+        v = [(torch.randn(npart, device="cuda", generator=g) * 0.7071).contiguous() for _ in range(3)]
+        mom = ctx.cell_moments(v[0], v[1], v[2], cs, 0)
+        coef = torch.zeros((ncell, 9), dtype=torch.float32, device="cuda")
+        flags = torch.zeros(ncell, dtype=torch.int32, device="cuda")
+        ts = []
+        for r in range(13):
+            flush.fill_(float(r))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fpcl.fp_closure_mlp(ctx.h, mom, 13, None, mlp, 0.2, coef, flags)
+            e1.record(); e1.synchronize()
+            if r >= 3:
+                ts.append(e0.elapsed_time(e1))
+        ms = float(np.median(ts))
+        useful = 2.0 * mac * ncell / (ms * 1e-3) / 1e12
+        res[name] = {"ms": ms, "cells_per_s": ncell / (ms * 1e-3), "useful_TFLOPs": useful,
+                     "roofline": {"bound": "tensor", "achieved": 3.0 * useful, "peak": bf16_peak, "unit": "TFLOP/s",
+                                  "frac": 3.0 * useful / bf16_peak,
+                                  "note": "achieved counts the three bf16 products executed per useful product; the "
+                                          "legacy mma.sync path tops out near 600 TFLOP/s on B200 (ncu "
+                                          "sm__ops_path_tensor_op_hmma peak 2048/clk/SM)"},
+                     "flagged_cells": int((flags != 0).sum().item())}
+        ctx.close()
+        del v, mom, coef, flags
+    return res
+
+
 def couette_small(fpcl, torch, workloads):
     """BASELINE config 1: 1D Couette, 50 cells x 100 particles, 100 fp_steps with the exact closure and again with the
     13-64-64-64-9 SiLU surrogate.  At 5,000 particles a step is nine kernel launches' worth of latency."""
@@ -579,6 +630,7 @@ def main():
         if not args.small:
             del a2, b2, out2
             extras["beyond_l2"] = corroborate(fpcl, torch, workloads, mlp_dev, hbm_peak, min(args.steps, 20))
+            extras["paper_surrogate_16_256x4_9"] = paper_surrogate(fpcl, torch, workloads, cfg["tau"])
             extras["c1_couette"] = couette_small(fpcl, torch, workloads)
             extras["c2_closure_microbench"] = closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak)
             extras["c4_ppc_sweep"] = ppc_sweep(fpcl, torch, workloads, 1000 if args.steps >= 100 else 100)
