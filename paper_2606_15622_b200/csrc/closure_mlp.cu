@@ -34,6 +34,7 @@ static inline int pad8(int v) { return (v + 7) & ~7; }
 
 #include "mlp_tc.cuh"
 #include "mlp_wide.cuh"
+#include "mlp_wide5.cuh"
 
 // repack caller weights [out][in] -> blob Wt[in][out_pad], bias[out_pad] (zero padded), scalers appended
 __global__ void mlp_pack_kernel(const __grid_constant__ mlp_desc D, const __grid_constant__ mlp_src S,
@@ -180,6 +181,7 @@ extern "C" int fp_set_mlp_tensor_cores(fp_ctx* ctx, int32_t enable)
 {
     if (!ctx) return FP_ERR_ARG;
     ctx->mlp_force_fp32 = (enable == 0);
+    ctx->mlp_wide_mma_sync = (enable == 2);
     return FP_OK;
 }
 
@@ -258,6 +260,40 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
     // ---- tensor-core path for wide networks [13|16]-256-...-256-9 (the paper's own shape, mlp_wide.cuh)
     bool wide = !ctx->mlp_force_fp32 && M.n_layers >= 2;
     for (int l = 1; l < M.n_layers && wide; ++l) wide = D.dims[l] == WD_H;
+    if (wide && !ctx->mlp_wide_mma_sync) {
+        // tcgen05 / TMEM kernel (mlp_wide5.cuh): weights as stage images + biases/scalers
+        const size_t bbytes = w5_blob_bytes(M.n_layers);
+        const size_t mbytes = (size_t)wd_misc_floats(M.n_layers) * sizeof(float);
+        if (C.w5_bytes < bbytes + mbytes) {
+            if (C.w5_blob) FP_CUDA_OK(ctx, cudaFree(C.w5_blob));
+            C.w5_blob = nullptr; C.w5_bytes = 0;
+            FP_CUDA_OK(ctx, cudaMalloc((void**)&C.w5_blob, bbytes + mbytes));
+            C.w5_bytes = bbytes + mbytes;
+        }
+        unsigned char* blob5 = reinterpret_cast<unsigned char*>(C.w5_blob);
+        float* misc = reinterpret_cast<float*>(blob5 + bbytes);
+        // biases and scalers come from the mma.sync pack kernel's misc section (same layout): pack both
+        fp_launch(mlpw5_pack_kernel, 2 * ctx->num_sms, 256, 0, st, S, M.n_layers, D.dims[0], reinterpret_cast<uint4*>(blob5));
+        fp_launch(mlpw_misc_kernel, 8, 256, 0, st, S, M.n_layers, D.dims[0], misc);
+        wd_params P;
+        P.stride = mom_stride; P.feature_set = M.feature_set; P.act = M.act; P.min_count = ctx->p.min_count_mlp;
+        P.ncell = ctx->ncell; P.nin = D.dims[0]; P.n_layers = M.n_layers; P.tau_scalar = ctx->p.tau;
+        P.n_scale = M.n_scale; P.theta_ref = M.theta_ref; P.relax_w = relax_w;
+        P.dt = ctx->p.dt; P.eps2_scale = ctx->p.eps2_scale; P.cellc = cellc;
+        const size_t smem = (size_t)2 * W5_A_PART + (size_t)W5_STAGES * W5_STAGE_BYTES +
+                            (size_t)((wd_misc_floats(M.n_layers) + 3) & ~3) * sizeof(float) + 16 * sizeof(uint64_t);
+        static bool attr5_set = false;
+        if (!attr5_set) {
+            FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_wide5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
+            attr5_set = true;
+        }
+        const int want = fp_div_up(ctx->ncell, W5_M);
+        fp_launch(mlp_wide5_kernel, want < ctx->num_sms ? want : ctx->num_sms, W5_THREADS, smem, st, mom, tau_cell,
+                  (const unsigned char*)blob5, (const float*)misc, coef, flags, P);
+        FP_LAUNCH_OK(ctx);
+        FP_COUNT(ctx, 3);
+        return FP_OK;
+    }
     if (wide) {
         const size_t fbytes = wd_frag_total(M.n_layers) * sizeof(uint4);
         const size_t mbytes = (size_t)wd_misc_floats(M.n_layers) * sizeof(float);

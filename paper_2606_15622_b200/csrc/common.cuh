@@ -30,6 +30,8 @@ struct fp_mlp_dev {                 // uploaded copy of the caller's MLP (fp_clo
     float*   tc_frags = nullptr;    // device: packed 3xTF32 mma fragments + biases/scalers (mlp_tc.cuh)
     float*   wd_frags = nullptr;    // device: packed split-bf16 mma fragments + biases/scalers (mlp_wide.cuh)
     size_t   wd_bytes = 0;
+    void*    w5_blob = nullptr;     // device: weights as tcgen05 stage images + biases/scalers (mlp_wide5.cuh)
+    size_t   w5_bytes = 0;
     float*   blob = nullptr;        // device: [W0 | b0 | W1 | b1 | ... | x_mean | x_scale | y_mean | y_scale]
     size_t   blob_floats = 0;
     size_t   w_off[FPCL_MAX_LAYERS] = {0}, b_off[FPCL_MAX_LAYERS] = {0};
@@ -71,6 +73,7 @@ struct fp_ctx {
     cudaEvent_t  ev_before_gather = nullptr, ev_after_gather = nullptr;
     fp_mlp_dev mlp;
     bool      mlp_force_fp32 = false;   // FPCL_MLP_FP32=1: always use the plain-FMA surrogate kernel
+    bool      mlp_wide_mma_sync = false;   // fp_set_mlp_tensor_cores(ctx, 2): wide networks on mma.sync instead of tcgen05
     // measurement hooks
     uint64_t  launches = 0;
     cudaEvent_t* t_ev = nullptr;     // [t_max * (FP_NSTAGES + 1)]

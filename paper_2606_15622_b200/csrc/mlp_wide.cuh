@@ -58,6 +58,24 @@ __device__ __forceinline__ void wd_mma(float (&c)[4], const uint32_t (&a)[4], ui
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
+__device__ __forceinline__ void wd_pack_misc(const mlp_src& S, int n_layers, int nin, float* __restrict__ misc, int tid, int nth)
+{
+    const int nm = wd_misc_floats(n_layers);
+    for (int e = tid; e < nm; e += nth) {
+        float v = 0.0f;
+        if (e < (n_layers - 1) * WD_H) v = S.b[e / WD_H][e % WD_H];
+        else if (e < (n_layers - 1) * WD_H + 16) { const int o = e - (n_layers - 1) * WD_H; v = (o < 9) ? S.b[n_layers - 1][o] : 0.0f; }
+        else {
+            const int q = (e - (n_layers - 1) * WD_H - 16) / 16, i = (e - (n_layers - 1) * WD_H - 16) % 16;
+            if (q == 0) v = (i < nin) ? S.x_mean[i] : 0.0f;
+            else if (q == 1) v = (i < nin) ? S.x_scale[i] : 1.0f;
+            else if (q == 2) v = (i < 9) ? S.y_mean[i] : 0.0f;
+            else v = (i < 9) ? S.y_scale[i] : 0.0f;
+        }
+        misc[e] = v;
+    }
+}
+
 // Pack caller weights W[l] ([out][in] row-major) into split bf16 mma B fragments.  Fragment (l, j, n, lane):
 // g = lane / 4, t = lane % 4, out = 8 n + g: b0 = inputs (16 j + 2 t, + 1), b1 = inputs (16 j + 2 t + 8, + 9).
 __global__ void mlpw_pack_kernel(const __grid_constant__ mlp_src S, int32_t n_layers, int32_t nin,
@@ -92,20 +110,14 @@ __global__ void mlpw_pack_kernel(const __grid_constant__ mlp_src S, int32_t n_la
         wd_split2(w[2], w[3], f.y, f.w);
         frags[e] = f;
     }
-    const int nm = wd_misc_floats(n_layers);
-    for (int e = (int)tid; e < nm; e += (int)nth) {
-        float v = 0.0f;
-        if (e < (n_layers - 1) * WD_H) v = S.b[e / WD_H][e % WD_H];
-        else if (e < (n_layers - 1) * WD_H + 16) { const int o = e - (n_layers - 1) * WD_H; v = (o < 9) ? S.b[n_layers - 1][o] : 0.0f; }
-        else {
-            const int q = (e - (n_layers - 1) * WD_H - 16) / 16, i = (e - (n_layers - 1) * WD_H - 16) % 16;
-            if (q == 0) v = (i < nin) ? S.x_mean[i] : 0.0f;
-            else if (q == 1) v = (i < nin) ? S.x_scale[i] : 1.0f;
-            else if (q == 2) v = (i < 9) ? S.y_mean[i] : 0.0f;
-            else v = (i < 9) ? S.y_scale[i] : 0.0f;
-        }
-        misc[e] = v;
-    }
+    wd_pack_misc(S, n_layers, nin, misc, (int)tid, (int)nth);
+}
+
+// biases and scalers alone (the tcgen05 kernel packs its weights differently, mlp_wide5.cuh)
+__global__ void mlpw_misc_kernel(const __grid_constant__ mlp_src S, int32_t n_layers, int32_t nin, float* __restrict__ misc)
+{
+    fpd_pdl();
+    wd_pack_misc(S, n_layers, nin, misc, (int)(blockIdx.x * blockDim.x + threadIdx.x), (int)(gridDim.x * blockDim.x));
 }
 
 #define WD_XS (WD_H + 8)                          // activation row stride in bf16 elements (528 bytes)

@@ -231,7 +231,7 @@ def fp_timing_read(ctx, max_steps):
 
 
 def fp_set_mlp_tensor_cores(ctx, enable):
-    _check(ctx, load().fp_set_mlp_tensor_cores(ctx, 1 if enable else 0), "fp_set_mlp_tensor_cores")
+    _check(ctx, load().fp_set_mlp_tensor_cores(ctx, int(enable)), "fp_set_mlp_tensor_cores")
 
 
 def fp_launch_count(ctx):

@@ -256,8 +256,9 @@ def test_closure_mlp(gpu, wl, orc, shape, stride):
     # the benchmark shape runs on the tensor cores by default (3xTF32: ~1e-5 of the output scale; north_star allows
     # 3e-3 for TF32); the plain fp32 kernel must meet 1e-5 for every shape, so it is checked as well
     # the paper's 16-256x4-9 network runs on the tensor cores too (mlp_wide.cuh: split-bf16 "3x" products)
-    variants = [("fp32", False, 1e-5)] + ([("tf32x3", True, 3e-5)] if shape.startswith(("13-64x3", "16-64x3")) else [])
-    variants += [("bf16x3", True, 1e-4)] if shape == "16-256x4-relu" else []
+    # (mode 1 = tcgen05/TMEM kernel mlp_wide5.cuh, mode 2 = mma.sync kernel mlp_wide.cuh)
+    variants = [("fp32", 0, 1e-5)] + ([("tf32x3", 1, 3e-5)] if shape.startswith(("13-64x3", "16-64x3")) else [])
+    variants += [("tcgen05 bf16x3", 1, 1e-4), ("mma.sync bf16x3", 2, 1e-4)] if shape == "16-256x4-relu" else []
     for vname, tc, tol in variants:
       gpu.fp_set_mlp_tensor_cores(ctx.h, tc)
       for relax_w in (1.0, 0.2):
