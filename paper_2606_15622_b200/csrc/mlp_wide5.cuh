@@ -11,15 +11,21 @@
 //     memory as the exact byte image of its stage (hi part, lo part, each canonical K-major), so a chunk is one copy;
 //   * one elected lane issues, per chunk, A_hi.B_hi, A_lo.B_hi, A_hi.B_lo and commits the stage back to the
 //     producer; after the last chunk of a layer it commits to the epilogue's barrier;
-//   * 4 epilogue warps (thread = cell): tcgen05.ld 32 columns at a time, + bias, activation, split, 16-byte stores
-//     of the next layer's A; the head (N = 16) ends in the de-standardisation, policy and blend of closure_mlp.cu.
-// Roles: warps 0-3 epilogue (and features), warp 4 producer, warp 5 mma issuer.  One CTA per SM, persistent over tiles.
+//   * 16 epilogue warps: accumulator -> + bias, activation, split -> 16-byte stores of the next layer's A, in
+//     32-column blocks; every finished block releases two k-steps of the next layer's mma, which accumulates into
+//     the other half of TMEM (2 x 256 columns), so the epilogue of layer l overlaps the mma of layer l + 1; the head
+//     (N = 16) ends in the de-standardisation, policy and blend of closure_mlp.cu.
+// Roles: warps 0-15 epilogue (warp w: TMEM lanes 32 (w % 4) .., columns 64 (w / 4) ..; warps 0-3 also compute the
+// features and finish the head), warp 16 producer, warp 17 mma issuer.  One CTA per SM, persistent over tiles.
 #pragma once
 #include <cuda_bf16.h>
 
-#define W5_THREADS 192
+#define W5_EPI_WARPS 16                           // 4 per TMEM lane quarter, each owns 64 of the 256 columns
+#define W5_THREADS ((W5_EPI_WARPS + 2) * 32)
 #define W5_M 128
+#ifndef W5_STAGES
 #define W5_STAGES 4
+#endif
 #define W5_STAGE_BYTES 16384                      // 256 units x 16 inputs x (hi + lo) bf16
 #define W5_A_PART (W5_M * WD_H * 2)               // 64 KB: one part (hi or lo) of the activations
 
@@ -74,6 +80,13 @@ __device__ __forceinline__ void w5_ld32(uint32_t taddr, uint32_t (&v)[32])
                    "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
                    "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
                    "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void w5_ld8(uint32_t taddr, uint32_t (&v)[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
                  : "r"(taddr) : "memory");
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
@@ -140,19 +153,19 @@ mlp_wide5_kernel(const double* __restrict__ mom, const float* __restrict__ tau_c
     uint64_t* bars = reinterpret_cast<uint64_t*>(ms + ((nmisc + 3) & ~3));
     uint64_t* full = bars;                       // [W5_STAGES] producer -> mma
     uint64_t* empty = bars + W5_STAGES;          // [W5_STAGES] mma -> producer
-    uint64_t* a_ready = bars + 2 * W5_STAGES;    // epilogue (128 arrivals) -> mma
-    uint64_t* d_ready = a_ready + 1;             // mma -> epilogue
+    uint64_t* a_blk = bars + 2 * W5_STAGES;      // [8] epilogue -> mma: 32-input block b of the next layer's A is written
+    uint64_t* d_ready = a_blk + 8;               // mma -> epilogue
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_ready + 1);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int L = P.n_layers;
     for (int i = tid; i < nmisc; i += W5_THREADS) ms[i] = misc[i];
     if (tid == 0) {
         for (int s = 0; s < W5_STAGES; ++s) { fpt_mbar_init(&full[s], 1); fpt_mbar_init(&empty[s], 1); }
-        fpt_mbar_init(a_ready, W5_M);
+        for (int b = 0; b < 8; ++b) fpt_mbar_init(&a_blk[b], W5_EPI_WARPS * 32);
         fpt_mbar_init(d_ready, 1);
     }
-    if (warp == 5) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(fpt_smem_u32(tmem_slot)), "r"(256u) : "memory");
+    if (warp == W5_EPI_WARPS + 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(fpt_smem_u32(tmem_slot)), "r"(512u) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     w5_fence_before();
@@ -162,7 +175,7 @@ mlp_wide5_kernel(const double* __restrict__ mom, const float* __restrict__ tau_c
     const int ntiles = (P.ncell + W5_M - 1) / W5_M;
     const int chunks_per_tile = 1 + (L - 2) * (WD_H / 16) + WD_H / 16;
 
-    if (warp == 4) {
+    if (warp == W5_EPI_WARPS) {
         // ===== producer: one lane streams the chunk sequence of every tile through the ring =====
         if (lane == 0) {
             uint32_t it = 0;
@@ -178,10 +191,10 @@ mlp_wide5_kernel(const double* __restrict__ mom, const float* __restrict__ tau_c
                 }
             }
         }
-    } else if (warp == 5) {
+    } else if (warp == W5_EPI_WARPS + 1) {
         // ===== mma issuer =====
         if (lane == 0) {
-            uint32_t it = 0, ar = 0;
+            uint32_t it = 0, ph0 = 0, ph1 = 0;          // completed phases of a_blk[0] and of a_blk[1..7]
             const uint32_t a_hi_s = fpt_smem_u32(a_hi), a_lo_s = fpt_smem_u32(a_lo), b_s = fpt_smem_u32(bst);
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 for (int l = 0; l < L; ++l) {
@@ -189,10 +202,12 @@ mlp_wide5_kernel(const double* __restrict__ mom, const float* __restrict__ tau_c
                     const int N = (l == L - 1) ? 16 : WD_H;
                     const uint32_t idesc = w5_idesc(N);
                     const uint32_t lbo_b = (uint32_t)(N / 8) * 128u, part_b = (uint32_t)N * 32u;
-                    w5_wait(a_ready, ar & 1u);
-                    ++ar;
-                    w5_fence_after();
+                    const uint32_t dcol = tmem + (uint32_t)(l & 1) * 256u;     // accumulators alternate between layers
                     for (int c = 0; c < nchunks; ++c, ++it) {
+                        if ((c & 1) == 0) {                  // inputs 16c .. 16c+31 = block c/2 of the producer's epilogue
+                            w5_wait(&a_blk[c >> 1], (c == 0 ? ph0 : ph1) & 1u);
+                            w5_fence_after();
+                        }
                         const uint32_t s = it % W5_STAGES, ph = (it / W5_STAGES) & 1u;
                         w5_wait(&full[s], ph);
                         w5_fence_after();
@@ -201,29 +216,32 @@ mlp_wide5_kernel(const double* __restrict__ mom, const float* __restrict__ tau_c
                         const uint64_t al = w5_desc(a_lo_s + (uint32_t)c * 4096u, 2048u, 128u);
                         const uint64_t bh = w5_desc(bb, lbo_b, 128u);
                         const uint64_t bl = w5_desc(bb + part_b, lbo_b, 128u);
-                        w5_mma(tmem, ah, bh, idesc, c > 0 ? 1u : 0u);
-                        w5_mma(tmem, al, bh, idesc, 1u);
-                        w5_mma(tmem, ah, bl, idesc, 1u);
+                        w5_mma(dcol, ah, bh, idesc, c > 0 ? 1u : 0u);
+                        w5_mma(dcol, al, bh, idesc, 1u);
+                        w5_mma(dcol, ah, bl, idesc, 1u);
                         w5_commit(&empty[s]);
                     }
+                    ++ph0;
+                    if (l > 0) ++ph1;
                     w5_commit(d_ready);
                 }
             }
         }
     } else {
-        // ===== epilogue warps: thread tid = row tid of the tile = TMEM lane tid =====
+        // ===== epilogue warps: row = TMEM lane 32 (warp % 4) + lane, columns 64 (warp / 4) .. + 63 =====
+        const int row = 32 * (warp & 3) + lane, cg = warp >> 2;
         const float* hbias = ms + (L - 1) * WD_H;
         const float* xmean = hbias + 16, *xscale = xmean + 16, *ymean = xscale + 16, *yscale = ymean + 16;
-        const uint32_t row_off = (uint32_t)(tid >> 3) * 128u + (uint32_t)(tid & 7) * 16u;   // inside an 8-input slab
-        const uint32_t tlane = tmem + ((uint32_t)(warp * 32) << 16);
+        const uint32_t row_off = (uint32_t)(row >> 3) * 128u + (uint32_t)(row & 7) * 16u;   // inside an 8-input slab
+        const uint32_t tlane = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
         uint32_t dr = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const int cell = tile * W5_M + tid;
-            const bool have = cell < P.ncell;
+            const int cell = tile * W5_M + row;
+            const bool have = cg == 0 && cell < P.ncell;
             double nraw = 0.0, theta = 0.0;
             float tau = P.tau_scalar;
             bool zbad = false;
-            {
+            if (cg == 0) {
                 float x[16];
 #pragma unroll
                 for (int i = 0; i < 16; ++i) x[i] = 0.0f;
@@ -268,44 +286,44 @@ mlp_wide5_kernel(const double* __restrict__ mom, const float* __restrict__ tau_c
                 *reinterpret_cast<uint4*>(a_lo + 2048 + row_off) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
             }
             fpt_fence_proxy_async();                      // generic-proxy stores -> visible to the tensor core's reads
-            w5_arrive(a_ready);
+            w5_arrive(&a_blk[0]);
             // ---- layers 0 .. L-2: accumulator -> bias, activation, split -> next layer's A (in place)
             for (int l = 0; l < L - 1; ++l) {
                 w5_wait(d_ready, dr & 1u);
                 ++dr;
                 w5_fence_after();
                 const float* bias = ms + l * WD_H;
+                const uint32_t dcol = tlane + (uint32_t)(l & 1) * 256u;
+                // 32-column blocks in order; the four warps of a row quarter take 8 columns each, and every finished
+                // block releases two k-steps of the next layer's mma (which writes the other accumulator)
 #pragma unroll 1
                 for (int cb = 0; cb < WD_H / 32; ++cb) {
-                    uint32_t v[32];
-                    w5_ld32(tlane + (uint32_t)(32 * cb), v);
+                    uint32_t v[8];
+                    w5_ld8(dcol + (uint32_t)(32 * cb + 8 * cg), v);
+                    uint32_t hi[4], lo[4];
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        uint32_t hi[4], lo[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const int c0 = 32 * cb + 8 * q + 2 * i;
-                            float s0 = __uint_as_float(v[8 * q + 2 * i]) + bias[c0];
-                            float s1 = __uint_as_float(v[8 * q + 2 * i + 1]) + bias[c0 + 1];
-                            s0 = (P.act == 0) ? __fdividef(s0, 1.0f + __expf(-s0)) : fmaxf(s0, 0.0f);
-                            s1 = (P.act == 0) ? __fdividef(s1, 1.0f + __expf(-s1)) : fmaxf(s1, 0.0f);
-                            wd_split2(s0, s1, hi[i], lo[i]);
-                        }
-                        const uint32_t o = (uint32_t)(4 * cb + q) * 2048u + row_off;
-                        *reinterpret_cast<uint4*>(a_hi + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-                        *reinterpret_cast<uint4*>(a_lo + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                    for (int i = 0; i < 4; ++i) {
+                        const int c0 = 32 * cb + 8 * cg + 2 * i;
+                        float s0 = __uint_as_float(v[2 * i]) + bias[c0];
+                        float s1 = __uint_as_float(v[2 * i + 1]) + bias[c0 + 1];
+                        s0 = (P.act == 0) ? __fdividef(s0, 1.0f + __expf(-s0)) : fmaxf(s0, 0.0f);
+                        s1 = (P.act == 0) ? __fdividef(s1, 1.0f + __expf(-s1)) : fmaxf(s1, 0.0f);
+                        wd_split2(s0, s1, hi[i], lo[i]);
                     }
+                    const uint32_t o = (uint32_t)(4 * cb + cg) * 2048u + row_off;
+                    *reinterpret_cast<uint4*>(a_hi + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+                    *reinterpret_cast<uint4*>(a_lo + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                    w5_fence_before();                    // the tcgen05.ld above is complete
+                    fpt_fence_proxy_async();
+                    w5_arrive(&a_blk[cb]);
                 }
-                w5_fence_before();                        // the tcgen05.ld above are complete
-                fpt_fence_proxy_async();
-                w5_arrive(a_ready);
             }
             // ---- head: 16 accumulator columns -> de-standardise, policy, blend
             w5_wait(d_ready, dr & 1u);
             ++dr;
             w5_fence_after();
             uint32_t yv[16];
-            w5_ld16(tlane, yv);
+            if (cg == 0) w5_ld16(tlane + (uint32_t)((L - 1) & 1) * 256u, yv);
             w5_fence_before();
             if (have) {
                 float y[9];
@@ -347,7 +365,7 @@ mlp_wide5_kernel(const double* __restrict__ mom, const float* __restrict__ tau_c
     // ---- teardown
     w5_fence_before();
     __syncthreads();
-    if (warp == 5) {
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(256u) : "memory");
+    if (warp == W5_EPI_WARPS + 1) {
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
     }
 }
