@@ -172,8 +172,13 @@ def _one_step(gpu, orc, cfg, st, closure, mlp, step_no, tau_fn=None, tau_ref_n=0
 
 
 @pytest.mark.parametrize("name", ["couette", "cavity", "cylinder"])
-@pytest.mark.parametrize("closure", [0, 1])
+@pytest.mark.parametrize("closure", [0, 1, 2])
 def test_step_one(gpu, wl, orc, name, closure):
+    # closure 2 = the surrogate step with the paper's own 16-256x4-9 network (tcgen05 kernel inside fp_step)
+    wide = closure == 2
+    if wide and name != "cavity":
+        pytest.skip("wide surrogate: cavity only")
+    closure = min(closure, 1)
     tau_fn, tau_ref_n = None, 0.0
     if name == "couette":
         cfg, st = wl.couette()
@@ -188,6 +193,9 @@ def test_step_one(gpu, wl, orc, name, closure):
             with np.errstate(divide="ignore"):
                 return np.where(N > 0, np.float32(tau_ref_n) / np.maximum(N, 1).astype(np.float32), tau_default).astype(np.float32)
     mlp = wl.xavier_mlp(n_scale=1.0 / 100.0, tau=cfg["tau"], bias_scale=0.1) if closure == 1 else None
+    if wide:
+        mlp = wl.xavier_mlp(dims=(16, 256, 256, 256, 256, 9), act=1, feature_set=1, n_scale=1.0 / 100.0, tau=cfg["tau"],
+                            bias_scale=0.1)
     got, res, ref, aux = _one_step(gpu, orc, cfg, st, closure, mlp, 3, tau_fn, tau_ref_n)
     # integer outputs: bit-exact
     assert np.array_equal(res["cell_start"], aux["cell_start"])
@@ -221,10 +229,10 @@ def test_step_one(gpu, wl, orc, name, closure):
     else:
         good = (aux["flags"] & orc.FLAG_EMPTY) == 0
         # benchmark-shape surrogate runs on the tensor cores (3xTF32, ~1e-5 of the output scale; see test_closure_mlp)
-        rc = coef_ratio(res["coef"], aux["coef"], tau, theta, 3e-5, mask=good)
+        rc = coef_ratio(res["coef"], aux["coef"], tau, theta, 1e-4 if wide else 3e-5, mask=good)
         # the surrogate standardises its inputs by 0.05-0.3, so at Mach 10 (|U| = 9) the ~1e-7 relative mismatch
         # of the two sides' moments reaches the coefficients at ~1e-5 and the velocities through (1 - E1) tau N
-        tolv = 5e-5 if name == "cylinder" else 4e-6
+        tolv = 5e-5 if name == "cylinder" else (1.5e-5 if wide else 4e-6)
     n = np.diff(aux["cell_start"])
     pm = np.repeat(good, n)
     cs_good = np.concatenate([[0], np.cumsum(n[good])]).astype(np.int64)
