@@ -239,7 +239,30 @@ def test_closure_exact_langevin(gpu, wl):
 
 
 # ------------------------------------------------------------------------------------------------ a5 MLP surrogate
-@pytest.mark.parametrize("shape", ["13-64x3-silu", "13-64x3-relu", "16-64x3-silu", "16-32-relu", "13-7-5-silu", "16-256x4-relu"])
+@pytest.mark.parametrize("nx,ny", [(1, 1), (50, 1), (43, 3), (16, 16)])
+def test_closure_mlp_wide_small_grids(gpu, wl, orc, nx, ny):
+    """Wide tensor-core kernels on grids of 1, 50, 129 and 256 cells (less than a tile, a ragged tile, exact tiles)."""
+    import torch
+    cfg, st = wl.ragged(nx=nx, ny=ny, seed=21, mean_ppc=60.0, empty_frac=0.0 if nx * ny == 1 else 0.1)
+    s, cs = _sorted_case(orc, cfg, st)
+    mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 0)
+    mlp = wl.xavier_mlp(dims=(16, 256, 256, 256, 256, 9), seed=0, act=1, feature_set=1, n_scale=1.0 / 60.0, tau=cfg["tau"],
+                        bias_scale=0.1)
+    tau = np.random.default_rng(3).uniform(0.4, 2.0, size=mom.shape[0]).astype(np.float32)
+    ctx = gpu.Context(cfg)
+    dm = gpu.Mlp(mlp)
+    ref, rflags = orc.closure_mlp(mom, mlp, tau, min_count=cfg["min_count_mlp"], relax_w=1.0, coef_old=None)
+    for mode in (1, 2):
+        gpu.fp_set_mlp_tensor_cores(ctx.h, mode)
+        coef, flags = ctx.closure_mlp(torch.from_numpy(mom).cuda(), dm, torch.from_numpy(tau).cuda(), 1.0)
+        coef, flags = coef.cpu().numpy(), flags.cpu().numpy().view(np.uint32)
+        assert np.array_equal(flags, rflags)
+        assert coef_ratio(coef, ref, tau, _theta(mom), 1e-4, mask=(rflags & orc.FLAG_EMPTY) == 0) <= 1.0
+    ctx.close()
+
+
+@pytest.mark.parametrize("shape", ["13-64x3-silu", "13-64x3-relu", "16-64x3-silu", "16-32-relu", "13-7-5-silu", "16-256x4-relu",
+                                   "13-256-silu", "16-256x7-relu"])
 @pytest.mark.parametrize("stride", [13, 29])
 def test_closure_mlp(gpu, wl, orc, shape, stride):
     import torch
@@ -248,7 +271,8 @@ def test_closure_mlp(gpu, wl, orc, shape, stride):
     mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 1 if stride == 29 else 0)
     dims, act, fs = {"13-64x3-silu": ((13, 64, 64, 64, 9), 0, 0), "13-64x3-relu": ((13, 64, 64, 64, 9), 1, 0), "16-64x3-silu": ((16, 64, 64, 64, 9), 0, 1),
                      "16-32-relu": ((16, 32, 9), 1, 1), "13-7-5-silu": ((13, 7, 5, 9), 0, 0),
-                     "16-256x4-relu": ((16, 256, 256, 256, 256, 9), 1, 1)}[shape]
+                     "16-256x4-relu": ((16, 256, 256, 256, 256, 9), 1, 1),
+                     "13-256-silu": ((13, 256, 9), 0, 0), "16-256x7-relu": ((16,) + (256,) * 7 + (9,), 1, 1)}[shape]
     mlp = wl.xavier_mlp(dims=dims, seed=0, act=act, feature_set=fs, n_scale=1.0 / 60.0, tau=cfg["tau"], bias_scale=0.1)
     tau = np.random.default_rng(3).uniform(0.4, 2.0, size=mom.shape[0]).astype(np.float32)
     ctx = gpu.Context(cfg)
@@ -258,7 +282,7 @@ def test_closure_mlp(gpu, wl, orc, shape, stride):
     # the paper's 16-256x4-9 network runs on the tensor cores too (mlp_wide.cuh: split-bf16 "3x" products)
     # (mode 1 = tcgen05/TMEM kernel mlp_wide5.cuh, mode 2 = mma.sync kernel mlp_wide.cuh)
     variants = [("fp32", 0, 1e-5)] + ([("tf32x3", 1, 3e-5)] if shape.startswith(("13-64x3", "16-64x3")) else [])
-    variants += [("tcgen05 bf16x3", 1, 1e-4), ("mma.sync bf16x3", 2, 1e-4)] if shape == "16-256x4-relu" else []
+    variants += [("tcgen05 bf16x3", 1, 1e-4), ("mma.sync bf16x3", 2, 1e-4)] if "-256" in shape else []
     for vname, tc, tol in variants:
       gpu.fp_set_mlp_tensor_cores(ctx.h, tc)
       for relax_w in (1.0, 0.2):
