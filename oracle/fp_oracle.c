@@ -18,7 +18,8 @@
  * brute-force Cramer, axis-permutation and scaling symmetries, Table 1 entries as printed; MLP -- hand cases,
  * parameter counts, independent numpy forward; Philox -- Random123 known-answer vectors and
  * numpy's Philox bit generator; update -- Eq. 15 identity, noise-off Langevin decay, conservation, OU
- * stationarity; walls -- half-range Maxwellian moments.
+ * stationarity; walls -- half-range Maxwellian moments; diagnostics -- hand values on octahedral ensembles, numpy
+ * slogdet, rotation invariance, Maxwellian limits.
  * Parity unpinned (no independent source exists): the value of eps^2 (R2-e), the low-count /
  * singular-cell policy (R3-c), the 16-feature definitions (R4), and the wall re-emission details (R7) as
  * compared with the paper's own runs.
@@ -294,6 +295,65 @@ void orc_closure_exact(int32_t ncell, const double *mom_full, const float *tau_c
         orc_closure_exact_cell(mom_full + (size_t)c * 29, tau, eps2_scale, min_count, coef + (size_t)c * 9,
                                flags + c, kappa ? kappa + c : NULL, NULL, NULL);
     }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-2: sampling outputs.
+ * Per-cell nonequilibrium diagnostics from the FULL record (R_ij = <c_i c_j c_k c_k>,
+ * Delta_4 = <(c_k c_k)^2> - 15 theta^2, theta = <c_k c_k>/3; Eq. 19-23 :632-657: Theta_ij = <c_i c_j>,
+ * D_G = -1/2 log det(Theta/theta), ds_eq = 3/2 log(theta/theta_inf) - log(rho/rho_inf),
+ * ds_kin,G = ds_eq - (D_G - D_G,inf), D_q = |q_hat|^2 / 5 with q_hat = <c |c|^2> / (2 theta^(3/2))).
+ * "norm" = divided by the local Maxwellian scale (reading R8: the paper only says
+ * "nondimensionalization by the corresponding local Maxwellian scales"): Delta_4 / (15 theta^2),
+ * R_ij / (5 theta^2) (a Maxwellian has <c_i c_j c^2> = 5 theta^2 delta_ij), sigma_norm = |P - theta I|_F / theta,
+ * q_norm = |q_hat|, m3_norm = |t|_F / theta^(3/2) (all 27 index triples).  DM6 = <(c^2)^3> needs a sixth-order
+ * accumulator that the FULL record does not carry and is not produced.
+ * diag record (16): theta, Delta_4, Delta_4/(15 theta^2), D_G, D_q, ds_eq, ds_kin,G, sigma_norm, q_norm, m3_norm,
+ *                   R_11, R_12, R_13, R_22, R_23, R_33 (each / (5 theta^2)).
+ * Empty cell or theta <= 0: zeros.  det(Theta/theta) <= 0 (fewer than 4 particles, or a degenerate cloud):
+ * D_G = +inf, ds_kin,G = -inf.  rho/rho_inf is N / n_inf (uniform particle weight).
+ * ------------------------------------------------------------------------------------------------ */
+void orc_cell_diagnostics(int32_t ncell, const double *mom_full, double theta_inf, double n_inf, double dg_inf,
+                          double *diag)
+{
+    static const double mult3[10] = {1, 3, 3, 3, 6, 3, 1, 3, 3, 1};       /* 111,112,113,122,123,133,222,223,233,333 */
+    for (int32_t cell = 0; cell < ncell; ++cell) {
+        const double *m = mom_full + (size_t)cell * 29;
+        double *d = diag + (size_t)cell * 16;
+        for (int k = 0; k < 16; ++k) d[k] = 0.0;
+        const double N = m[0];
+        const double *P = m + 4, *t = m + 10, *F = m + 20;
+        const double theta = (P[0] + P[3] + P[5]) / 3.0;
+        if (!(N > 0.0) || !(theta > 0.0)) continue;
+        const double c4 = F[0] + F[3] + F[5];                              /* <c^4> = F_kk */
+        d[0] = theta;
+        d[1] = c4 - 15.0 * theta * theta;
+        d[2] = d[1] / (15.0 * theta * theta);
+        const double a = P[0] / theta, b = P[1] / theta, c = P[2] / theta, e = P[3] / theta, f = P[4] / theta,
+                     g = P[5] / theta;                                     /* Theta/theta = [[a,b,c],[b,e,f],[c,f,g]] */
+        const double det = a * (e * g - f * f) - b * (b * g - f * c) + c * (b * f - e * c);
+        d[3] = det > 0.0 ? -0.5 * log(det) : INFINITY;
+        double h[3];
+        orc_record_h(m, 29, h);
+        const double qn = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]) / (2.0 * theta * sqrt(theta));
+        d[4] = qn * qn / 5.0;
+        d[5] = 1.5 * log(theta / theta_inf) - log(N / n_inf);
+        d[6] = d[5] - (d[3] - dg_inf);
+        const double sxx = P[0] - theta, syy = P[3] - theta, szz = P[5] - theta;
+        d[7] = sqrt(sxx * sxx + syy * syy + szz * szz + 2.0 * (P[1] * P[1] + P[2] * P[2] + P[4] * P[4])) / theta;
+        d[8] = qn;
+        double t2 = 0.0;
+        for (int k = 0; k < 10; ++k) t2 += mult3[k] * t[k] * t[k];
+        d[9] = sqrt(t2) / (theta * sqrt(theta));
+        for (int k = 0; k < 6; ++k) d[10 + k] = F[k] / (5.0 * theta * theta);
+    }
+}
+
+/* Running time average of sampled grid fields (PAPER.md:217-219 average_results): after the call avg holds the
+ * mean of the k + 1 samples seen so far, avg <- avg + (x - avg) / (k + 1). */
+void orc_average_results(int64_t n, const double *x, int64_t k, double *avg)
+{
+    for (int64_t i = 0; i < n; ++i) avg[i] = avg[i] + (x[i] - avg[i]) / (double)(k + 1);
 }
 
 /* ------------------------------------------------------------------------------------------------

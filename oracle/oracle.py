@@ -97,6 +97,25 @@ def cell_moments(vx, vy, vz, cell_start, mode):
     return mom
 
 
+def cell_diagnostics(mom_full, theta_inf=0.5, n_inf=1.0, dg_inf=0.0):
+    """NEXT-2: 16 diagnostics per cell from the FULL record (fp_oracle.c orc_cell_diagnostics)."""
+    mom_full = _f64(mom_full)
+    ncell = mom_full.shape[0]
+    assert mom_full.shape[1] == 29
+    diag = np.empty((ncell, 16), dtype=np.float64)
+    lib().orc_cell_diagnostics(C.c_int32(ncell), _p(mom_full, C.c_double), C.c_double(theta_inf), C.c_double(n_inf),
+                               C.c_double(dg_inf), _p(diag, C.c_double))
+    return diag
+
+
+def average_results(x, k, avg):
+    """NEXT-2: running mean, in place on avg."""
+    x = _f64(x)
+    assert avg.dtype == np.float64 and avg.flags["C_CONTIGUOUS"] and avg.size == x.size
+    lib().orc_average_results(C.c_int64(x.size), _p(x, C.c_double), C.c_int64(k), _p(avg, C.c_double))
+    return avg
+
+
 # ---------------------------------------------------------------- S2/S3
 def _tau_args(tau, ncell):
     if np.ndim(tau) == 0:
