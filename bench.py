@@ -177,6 +177,7 @@ def algorithmic_bytes(np_, ncell):
         "closure_mlp": 144 * ncell,                        # 104 r + 36 w + 4 w
         "update": 28 * np_ + (4 + 232 + 36 + 4) * ncell,   # 12 r + 4 r pid + 12 w; per cell start, record, coef, flags
         "update_lite": 28 * np_ + (4 + 104 + 36 + 4) * ncell,
+        "cell_diagnostics": (232 + 128) * ncell,           # FULL record read, 16 doubles written (NEXT-2)
         "gather": 52 * np_,                                # 4 r perm + 24 r + 24 w
         "sort_keys": 36 * np_,                             # 2 passes x (4+4 r hist+scatter keys) + idx r/w
     }
@@ -219,6 +220,9 @@ def cold_kernel_table(fpcl, torch, ctx, state, out, mlp_dev, hbm_peak, reps=20):
     res["moments_lite"] = timed(lambda r: ctx.cell_moments(v[0], v[1], v[2], cs, 0, out=mom_lite), "moments_lite")
     res["closure_exact"] = timed(lambda r: fpcl.fp_closure_exact(ctx.h, mom_full, None, coef, flags), "closure_exact")
     res["closure_exact"]["cells_per_s"] = ncell / (res["closure_exact"]["ms"] * 1e-3)
+    diag = torch.empty((ncell, 16), dtype=torch.float64, device="cuda")
+    res["cell_diagnostics"] = timed(lambda r: ctx.cell_diagnostics(mom_full, 0.5, 100.0, 0.0, out=diag), "cell_diagnostics")
+    res["cell_diagnostics"]["cells_per_s"] = ncell / (res["cell_diagnostics"]["ms"] * 1e-3)
     if mlp_dev is not None:
         res["closure_mlp"] = timed(lambda r: fpcl.fp_closure_mlp(ctx.h, mom_lite, 13, None, mlp_dev, 1.0, coef, flags),
                                    "closure_mlp")

@@ -147,6 +147,21 @@ int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const flo
  * under any setting.  The environment variable FPCL_MLP_FP32=1 sets enable = 0 at fp_create. */
 int fp_set_mlp_tensor_cores(fp_ctx* ctx, int32_t enable);
 
+/* Sampling outputs (they run once per sampled step, outside the per-step path).
+ * fp_cell_diagnostics: 16 fp64 values per cell from the FULL record (PAPER.md:415 and Eq. 19-23 :632-657; the
+ * normalisations are reading R8 of DESIGN.md): theta = P_kk/3; Delta_4 = <c^4> - 15 theta^2; Delta_4/(15 theta^2);
+ * D_G = -1/2 log det(P/theta); D_q = |q_hat|^2/5 with q_hat = h/(2 theta^1.5); ds_eq = 3/2 log(theta/theta_inf) -
+ * log(N/n_inf); ds_kin,G = ds_eq - (D_G - dg_inf); sigma_norm = |P - theta I|_F/theta; q_norm = |q_hat|;
+ * m3_norm = |t|_F/theta^1.5; R_11, R_12, R_13, R_22, R_23, R_33, each <c_i c_j c^2>/(5 theta^2).  Empty or cold
+ * (theta <= 0) cell: zeros; singular covariance (N < 4, or det <= 0): D_G = +inf, ds_kin,G = -inf.  DM6 needs a sixth-order
+ * sum the record does not carry and is not produced.  mom_full [ncell*29], diag [ncell*16] (16-byte aligned),
+ * device memory; theta_inf, n_inf > 0 are the upstream reference state (Eq. 20), dg_inf its D_G (Eq. 23).
+ * fp_average_results: running time average, avg[i] <- avg[i] + (x[i] - avg[i])/(k + 1) for
+ * i < n, k = number of samples already averaged; x, avg device fp64. */
+int fp_cell_diagnostics(fp_ctx* ctx, const double* mom_full, double theta_inf, double n_inf, double dg_inf,
+                        double* diag, void* stream);
+int fp_average_results(fp_ctx* ctx, int64_t n, const double* x, int64_t k, double* avg, void* stream);
+
 /* a6 -- FP velocity update, in place on cell-sorted vx, vy, vz (Eq. 13-15 :150-181; R5, R6).
  * step is the Philox counter word for time.  flags [ncell] are OR-ed with FP_FLAG_ALPHA / FP_FLAG_SKIPPED. */
 int fp_velocity_update(fp_ctx* ctx, int64_t np, float* vx, float* vy, float* vz, const uint32_t* pid,

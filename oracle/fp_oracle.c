@@ -310,8 +310,9 @@ void orc_closure_exact(int32_t ncell, const double *mom_full, const float *tau_c
  * accumulator that the FULL record does not carry and is not produced.
  * diag record (16): theta, Delta_4, Delta_4/(15 theta^2), D_G, D_q, ds_eq, ds_kin,G, sigma_norm, q_norm, m3_norm,
  *                   R_11, R_12, R_13, R_22, R_23, R_33 (each / (5 theta^2)).
- * Empty cell or theta <= 0: zeros.  det(Theta/theta) <= 0 (fewer than 4 particles, or a degenerate cloud):
- * D_G = +inf, ds_kin,G = -inf.  rho/rho_inf is N / n_inf (uniform particle weight).
+ * Empty cell or theta <= 0: zeros.  Singular covariance: D_G = +inf, ds_kin,G = -inf; "singular" is N < 4 (the
+ * covariance of N points has rank <= N - 1, its determinant is zero up to rounding, and the sign of that rounding
+ * must not decide the result) or det(Theta/theta) <= 0 (a degenerate cloud).  rho/rho_inf is N / n_inf (uniform particle weight).
  * ------------------------------------------------------------------------------------------------ */
 void orc_cell_diagnostics(int32_t ncell, const double *mom_full, double theta_inf, double n_inf, double dg_inf,
                           double *diag)
@@ -332,7 +333,7 @@ void orc_cell_diagnostics(int32_t ncell, const double *mom_full, double theta_in
         const double a = P[0] / theta, b = P[1] / theta, c = P[2] / theta, e = P[3] / theta, f = P[4] / theta,
                      g = P[5] / theta;                                     /* Theta/theta = [[a,b,c],[b,e,f],[c,f,g]] */
         const double det = a * (e * g - f * f) - b * (b * g - f * c) + c * (b * f - e * c);
-        d[3] = det > 0.0 ? -0.5 * log(det) : INFINITY;
+        d[3] = (N >= 4.0 && det > 0.0) ? -0.5 * log(det) : INFINITY;
         double h[3];
         orc_record_h(m, 29, h);
         const double qn = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]) / (2.0 * theta * sqrt(theta));

@@ -19,7 +19,8 @@ FLAG_EMPTY, FLAG_LOWCOUNT, FLAG_SINGULAR, FLAG_ILLCOND, FLAG_ALPHA, FLAG_SKIPPED
 
 EXPORTS = ["fp_create", "fp_destroy", "fp_last_error", "fp_version", "fp_sort_by_cell", "fp_cell_moments",
            "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host",
-           "fp_timing_enable", "fp_timing_read", "fp_launch_count", "fp_set_mlp_tensor_cores"]
+           "fp_timing_enable", "fp_timing_read", "fp_launch_count", "fp_set_mlp_tensor_cores", "fp_cell_diagnostics",
+           "fp_average_results"]
 NSTAGES = 6
 STAGE_NAMES = ["stream_walls", "sort_keys", "gather", "moments", "closure", "update"]
 
@@ -71,6 +72,8 @@ def load(path=None):
     lib.fp_closure_exact.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.fp_closure_mlp.argtypes = [vp, vp, i32, vp, C.POINTER(FpMlp), f32, vp, vp, vp]
     lib.fp_velocity_update.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, u64, vp, vp]
+    lib.fp_cell_diagnostics.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, vp, vp]
+    lib.fp_average_results.argtypes = [vp, i64, vp, i64, vp, vp]
     lib.fp_stream_walls.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, u64, vp]
     lib.fp_step.argtypes = [vp, i64] + [vp] * 12 + [i32, C.POINTER(FpMlp), f32, i32, f32, vp, u64, vp, vp, vp, vp, vp]
     lib.fp_step_host.argtypes = [vp, i64] + [vp] * 6 + [i32, C.POINTER(FpMlp), f32, u64, vp, vp, vp, vp]
@@ -179,6 +182,16 @@ def fp_velocity_update(ctx, np_, vx, vy, vz, pid, cell_start, mom, mom_stride, c
                                           _ptr(pid, torch.int32, np_), _ptr(cell_start, torch.int32),
                                           _ptr(mom, torch.float64), mom_stride, _ptr(coef, f), _ptr(tau_cell, f),
                                           step, _ptr(flags, torch.int32), _stream()), "fp_velocity_update")
+
+
+def fp_cell_diagnostics(ctx, mom_full, theta_inf, n_inf, dg_inf, diag):
+    _check(ctx, load().fp_cell_diagnostics(ctx, _ptr(mom_full, torch.float64), float(theta_inf), float(n_inf),
+                                           float(dg_inf), _ptr(diag, torch.float64), _stream()), "fp_cell_diagnostics")
+
+
+def fp_average_results(ctx, x, k, avg):
+    _check(ctx, load().fp_average_results(ctx, x.numel(), _ptr(x, torch.float64), int(k),
+                                          _ptr(avg, torch.float64, x.numel()), _stream()), "fp_average_results")
 
 
 def fp_stream_walls(ctx, np_, x, y, vx, vy, vz, pid, step):
@@ -335,6 +348,11 @@ class Context:
         flags = torch.empty(self.ncell, dtype=torch.int32, device=self.device)
         fp_closure_mlp(self.h, mom, mom.shape[1], tau_cell, mlp, relax_w, coef, flags)
         return coef, flags
+
+    def cell_diagnostics(self, mom_full, theta_inf=0.5, n_inf=1.0, dg_inf=0.0, out=None):
+        diag = out if out is not None else torch.empty((self.ncell, 16), dtype=torch.float64, device=self.device)
+        fp_cell_diagnostics(self.h, mom_full, theta_inf, n_inf, dg_inf, diag)
+        return diag
 
     def velocity_update(self, vx, vy, vz, pid, cell_start, mom, coef, step, flags, tau_cell=None):
         fp_velocity_update(self.h, vx.numel(), vx, vy, vz, pid, cell_start, mom, mom.shape[1], coef, tau_cell, step,

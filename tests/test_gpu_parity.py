@@ -297,3 +297,36 @@ def test_closure_mlp(gpu, wl, orc, shape, stride):
           assert r <= 1.0
           assert np.isfinite(coef).all()
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-2 sampling outputs
+def test_cell_diagnostics_and_average(gpu, wl, orc):
+    """fp_cell_diagnostics / fp_average_results vs the oracle on a ragged grid (empty, 1-, 2-, 3-particle cells give
+    zeros / +inf the same way on both sides); fp64 on both sides: 1e-12 relative to each value's scale."""
+    import torch
+    cfg, st = wl.ragged(nx=37, ny=23, seed=17, mean_ppc=40.0)
+    s, cs = _sorted_case(orc, cfg, st)
+    mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 1)
+    ref = orc.cell_diagnostics(mom, theta_inf=0.45, n_inf=37.0, dg_inf=0.02)
+    ctx = gpu.Context(cfg)
+    got = ctx.cell_diagnostics(torch.from_numpy(mom).cuda(), 0.45, 37.0, 0.02).cpu().numpy()
+    assert np.array_equal(np.isinf(got), np.isinf(ref)) and np.array_equal(np.sign(got[np.isinf(ref)]), np.sign(ref[np.isinf(ref)]))
+    fin = np.isfinite(ref)
+    assert np.isfinite(got[fin]).all()
+    # D_G and the entropies come from log det of a matrix near the identity: compare absolutely there
+    err = np.abs(got[fin] - ref[fin]) / (1.0 + np.abs(ref[fin]))
+    print("cell_diagnostics: max err %.3g over %d cells (%d singular)" % (err.max(), mom.shape[0], int(np.isinf(ref[:, 3]).sum())))
+    assert err.max() < 1e-12
+    n = np.diff(cs)
+    assert (got[n == 0] == 0).all()
+    # running average over 5 samples of the record itself
+    rng = np.random.default_rng(4)
+    avg_ref = np.zeros_like(mom)
+    avg = torch.zeros(mom.shape, dtype=torch.float64, device="cuda")
+    for k in range(5):
+        x = mom * rng.uniform(0.5, 1.5, size=mom.shape)
+        orc.average_results(x, k, avg_ref)
+        gpu.fp_average_results(ctx.h, torch.from_numpy(x).cuda(), k, avg)
+    a = avg.cpu().numpy()
+    assert np.allclose(a, avg_ref, rtol=1e-14, atol=1e-300)
+    ctx.close()
