@@ -350,6 +350,28 @@ void orc_cell_diagnostics(int32_t ncell, const double *mom_full, double theta_in
     }
 }
 
+/* DM6 = <(c_k c_k)^3>, the sixth central moment of PAPER.md:415, per cell from the cell-sorted particles (the FULL
+ * record stops at fifth order).  dm6[cell] = (1/N) sum (|v - U|^2)^3 with U the cell mean (recomputed here); empty
+ * cell: 0.  A Maxwellian has <c^6> = 105 theta^3, which is the "local Maxwellian scale" of DM6_norm (reading R8). */
+void orc_cell_dm6(const float *vx, const float *vy, const float *vz, const int32_t *cell_start, int32_t ncell, double *dm6)
+{
+    for (int32_t cell = 0; cell < ncell; ++cell) {
+        int64_t s = cell_start[cell], e = cell_start[cell + 1], n = e - s;
+        dm6[cell] = 0.0;
+        if (n <= 0) continue;
+        double U[3] = {0, 0, 0};
+        for (int64_t p = s; p < e; ++p) { U[0] += vx[p]; U[1] += vy[p]; U[2] += vz[p]; }
+        for (int i = 0; i < 3; ++i) U[i] /= (double)n;
+        double acc = 0.0;
+        for (int64_t p = s; p < e; ++p) {
+            double c0 = (double)vx[p] - U[0], c1 = (double)vy[p] - U[1], c2 = (double)vz[p] - U[2];
+            double r2 = c0 * c0 + c1 * c1 + c2 * c2;
+            acc += r2 * r2 * r2;
+        }
+        dm6[cell] = acc / (double)n;
+    }
+}
+
 /* Running time average of sampled grid fields (PAPER.md:217-219 average_results): after the call avg holds the
  * mean of the k + 1 samples seen so far, avg <- avg + (x - avg) / (k + 1). */
 void orc_average_results(int64_t n, const double *x, int64_t k, double *avg)

@@ -108,6 +108,16 @@ def cell_diagnostics(mom_full, theta_inf=0.5, n_inf=1.0, dg_inf=0.0):
     return diag
 
 
+def cell_dm6(vx, vy, vz, cell_start):
+    """NEXT-2: DM6 = <(c^2)^3> per cell."""
+    vx, vy, vz, cell_start = _f32(vx), _f32(vy), _f32(vz), _i32(cell_start)
+    ncell = cell_start.shape[0] - 1
+    dm6 = np.empty(ncell, dtype=np.float64)
+    lib().orc_cell_dm6(_p(vx, C.c_float), _p(vy, C.c_float), _p(vz, C.c_float), _p(cell_start, C.c_int32),
+                       C.c_int32(ncell), _p(dm6, C.c_double))
+    return dm6
+
+
 def average_results(x, k, avg):
     """NEXT-2: running mean, in place on avg."""
     x = _f64(x)

@@ -129,3 +129,22 @@ def test_running_average_is_the_mean(orc):
     for k in range(7):
         orc.average_results(xs[k], k, avg)
         assert np.allclose(avg, xs[: k + 1].mean(axis=0), rtol=1e-13, atol=1e-15)
+
+
+def test_dm6_hand_and_maxwellian(orc):
+    # octahedron: every particle has c^2 = a^2 -> DM6 = a^6 exactly (any bulk velocity);  2 + 4 points on a line:
+    # c = 2a (x2), -a (x4): <c^6> = (2 * 64 + 4) / 6 a^6 = 22 a^6;  Maxwellian: <c^6> = 105 theta^3 (chi-square with 3
+    # degrees of freedom: E[r^6] = 3 * 5 * 7 theta^3)
+    a = 1.5
+    v = _octa(a, a, a, shift=(3.0, 0.25, -7.0)).astype(np.float32)
+    cs = np.array([0, 6], dtype=np.int32)
+    assert orc.cell_dm6(v[:, 0], v[:, 1], v[:, 2], cs)[0] == pytest.approx(a ** 6, rel=1e-6)
+    b = 0.5
+    w = np.array([[2 * b, 0, 0]] * 2 + [[-b, 0, 0]] * 4, dtype=np.float32)
+    assert orc.cell_dm6(w[:, 0], w[:, 1], w[:, 2], cs)[0] == pytest.approx(22 * b ** 6, rel=1e-6)
+    rng = np.random.default_rng(3)
+    n = 400000
+    g = (rng.normal(scale=np.sqrt(0.5), size=(n, 3)) + np.array([1.0, 2.0, -3.0])).astype(np.float32)
+    got = orc.cell_dm6(g[:, 0], g[:, 1], g[:, 2], np.array([0, 0, n], dtype=np.int32))
+    assert got[0] == 0.0                                            # empty cell
+    assert got[1] == pytest.approx(105 * 0.5 ** 3, rel=0.03)        # relative sd of the estimate ~ 10 / sqrt(n)
