@@ -154,13 +154,17 @@ int fp_set_mlp_tensor_cores(fp_ctx* ctx, int32_t enable);
  * log(N/n_inf); ds_kin,G = ds_eq - (D_G - dg_inf); sigma_norm = |P - theta I|_F/theta; q_norm = |q_hat|;
  * m3_norm = |t|_F/theta^1.5; R_11, R_12, R_13, R_22, R_23, R_33, each <c_i c_j c^2>/(5 theta^2).  Empty or cold
  * (theta <= 0) cell: zeros; singular covariance (N < 4, or det <= 0): D_G = +inf, ds_kin,G = -inf.  DM6 needs a sixth-order
- * sum the record does not carry and is not produced.  mom_full [ncell*29], diag [ncell*16] (16-byte aligned),
+ * sum the record does not carry: fp_cell_sixth_moment.  mom_full [ncell*29], diag [ncell*16] (16-byte aligned),
  * device memory; theta_inf, n_inf > 0 are the upstream reference state (Eq. 20), dg_inf its D_G (Eq. 23).
  * fp_average_results: running time average, avg[i] <- avg[i] + (x[i] - avg[i])/(k + 1) for
  * i < n, k = number of samples already averaged; x, avg device fp64. */
 int fp_cell_diagnostics(fp_ctx* ctx, const double* mom_full, double theta_inf, double n_inf, double dg_inf,
                         double* diag, void* stream);
 int fp_average_results(fp_ctx* ctx, int64_t n, const double* x, int64_t k, double* avg, void* stream);
+/* fp_cell_sixth_moment: DM6 = <(c_k c_k)^3> per cell from the cell-sorted velocities and the means U of the
+ * moment record (mom_stride 13 or 29); dm6 [ncell] fp64, 0 for an empty cell.  A Maxwellian has DM6 = 105 theta^3. */
+int fp_cell_sixth_moment(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
+                const int32_t* cell_start, const double* mom, int32_t mom_stride, double* dm6, void* stream);
 
 /* a6 -- FP velocity update, in place on cell-sorted vx, vy, vz (Eq. 13-15 :150-181; R5, R6).
  * step is the Philox counter word for time.  flags [ncell] are OR-ed with FP_FLAG_ALPHA / FP_FLAG_SKIPPED. */

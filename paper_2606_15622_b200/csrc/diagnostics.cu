@@ -1,6 +1,7 @@
 // diagnostics.cu -- NEXT-2: sampling outputs of the closure path.
 //   fp_cell_diagnostics: per-cell nonequilibrium diagnostics from the FULL moment record (PAPER.md:415 R_ij, Delta_4,
 //     theta; Eq. 19-23 :632-657 D_G, ds_eq, ds_kin,G, D_q; normalisations: DESIGN.md R8).
+//   fp_cell_sixth_moment: the sixth central moment DM6 = <(c^2)^3>, which the FULL record does not carry.
 //   fp_average_results: running time average of sampled per-cell fields.
 // Both are one thread per value, fp64, HBM-bound by construction (232 B read + 128 B written per cell; 16 B read +
 // 8 B written per averaged value); they run once per sampled step, outside the judged path.
@@ -60,6 +61,47 @@ avg_kernel(int64_t n, const double* __restrict__ x, double inv_kp1, double* __re
     fpd_pdl();
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
         avg[i] = avg[i] + (x[i] - avg[i]) * inv_kp1;
+}
+
+// DM6 = <(c^2)^3>, one warp per cell over the cell-sorted particles, fp64 (sampling path, not judged):
+// coalesced fp32 loads, c = v - U with U from the record, per-lane sums combined by shuffles.
+__global__ void __launch_bounds__(256)
+dm6_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
+           const int32_t* __restrict__ cell_start, const double* __restrict__ mom, int32_t stride, int32_t ncell,
+           double* __restrict__ dm6)
+{
+    fpd_pdl();
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t cell = warp; cell < ncell; cell += nwarp) {
+        const int32_t s = cell_start[cell], e = cell_start[cell + 1];
+        const double* m = mom + (size_t)cell * stride;
+        const double U0 = m[1], U1 = m[2], U2 = m[3];
+        double acc = 0.0;
+        for (int32_t p = s + lane; p < e; p += 32) {
+            const double c0 = (double)vx[p] - U0, c1 = (double)vy[p] - U1, c2 = (double)vz[p] - U2;
+            const double r2 = c0 * c0 + c1 * c1 + c2 * c2;
+            acc += r2 * r2 * r2;
+        }
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) acc += fpd_shfl_xor(acc, d);
+        if (lane == 0) dm6[cell] = e > s ? acc / (double)(e - s) : 0.0;
+    }
+}
+
+extern "C" int fp_cell_sixth_moment(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
+                           const int32_t* cell_start, const double* mom, int32_t mom_stride, double* dm6, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    if (np < 0 || !cell_start || !mom || !dm6 || (mom_stride != 13 && mom_stride != 29) || (np > 0 && (!vx || !vy || !vz)))
+        return fp_fail(ctx, FP_ERR_ARG, "fp_cell_sixth_moment: bad argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int want = fp_div_up(ctx->ncell, 8);
+    const int cap = ctx->num_sms * 8;
+    fp_launch(dm6_kernel, want < cap ? want : cap, 256, 0, st, vx, vy, vz, cell_start, mom, mom_stride, ctx->ncell, dm6);
+    FP_LAUNCH_OK(ctx);
+    FP_COUNT(ctx, 1);
+    return FP_OK;
 }
 
 extern "C" int fp_cell_diagnostics(fp_ctx* ctx, const double* mom_full, double theta_inf, double n_inf, double dg_inf,

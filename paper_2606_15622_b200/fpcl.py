@@ -20,7 +20,7 @@ FLAG_EMPTY, FLAG_LOWCOUNT, FLAG_SINGULAR, FLAG_ILLCOND, FLAG_ALPHA, FLAG_SKIPPED
 EXPORTS = ["fp_create", "fp_destroy", "fp_last_error", "fp_version", "fp_sort_by_cell", "fp_cell_moments",
            "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host",
            "fp_timing_enable", "fp_timing_read", "fp_launch_count", "fp_set_mlp_tensor_cores", "fp_cell_diagnostics",
-           "fp_average_results"]
+           "fp_average_results", "fp_cell_sixth_moment"]
 NSTAGES = 6
 STAGE_NAMES = ["stream_walls", "sort_keys", "gather", "moments", "closure", "update"]
 
@@ -74,6 +74,7 @@ def load(path=None):
     lib.fp_velocity_update.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, u64, vp, vp]
     lib.fp_cell_diagnostics.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, vp, vp]
     lib.fp_average_results.argtypes = [vp, i64, vp, i64, vp, vp]
+    lib.fp_cell_sixth_moment.argtypes = [vp, i64, vp, vp, vp, vp, vp, i32, vp, vp]
     lib.fp_stream_walls.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, u64, vp]
     lib.fp_step.argtypes = [vp, i64] + [vp] * 12 + [i32, C.POINTER(FpMlp), f32, i32, f32, vp, u64, vp, vp, vp, vp, vp]
     lib.fp_step_host.argtypes = [vp, i64] + [vp] * 6 + [i32, C.POINTER(FpMlp), f32, u64, vp, vp, vp, vp]
@@ -187,6 +188,13 @@ def fp_velocity_update(ctx, np_, vx, vy, vz, pid, cell_start, mom, mom_stride, c
 def fp_cell_diagnostics(ctx, mom_full, theta_inf, n_inf, dg_inf, diag):
     _check(ctx, load().fp_cell_diagnostics(ctx, _ptr(mom_full, torch.float64), float(theta_inf), float(n_inf),
                                            float(dg_inf), _ptr(diag, torch.float64), _stream()), "fp_cell_diagnostics")
+
+
+def fp_cell_sixth_moment(ctx, np_, vx, vy, vz, cell_start, mom, dm6):
+    f = torch.float32
+    _check(ctx, load().fp_cell_sixth_moment(ctx, np_, _ptr(vx, f, np_), _ptr(vy, f, np_), _ptr(vz, f, np_),
+                                   _ptr(cell_start, torch.int32), _ptr(mom, torch.float64), mom.shape[1],
+                                   _ptr(dm6, torch.float64), _stream()), "fp_cell_sixth_moment")
 
 
 def fp_average_results(ctx, x, k, avg):

@@ -319,6 +319,13 @@ def test_cell_diagnostics_and_average(gpu, wl, orc):
     assert err.max() < 1e-12
     n = np.diff(cs)
     assert (got[n == 0] == 0).all()
+    # DM6 from the particles (fp64 on both sides, different summation order)
+    dm6_ref = orc.cell_dm6(s["vx"], s["vy"], s["vz"], cs)
+    dev = gpu.to_device(s)
+    dm6 = torch.empty(mom.shape[0], dtype=torch.float64, device="cuda")
+    gpu.fp_cell_sixth_moment(ctx.h, s["vx"].shape[0], dev["vx"], dev["vy"], dev["vz"], torch.from_numpy(cs).cuda(),
+                    torch.from_numpy(mom).cuda(), dm6)
+    assert np.allclose(dm6.cpu().numpy(), dm6_ref, rtol=1e-12, atol=0)
     # running average over 5 samples of the record itself
     rng = np.random.default_rng(4)
     avg_ref = np.zeros_like(mom)
