@@ -168,6 +168,20 @@ def test_moments_group_widths(gpu, wl, orc):
             print("moments ppc %g mode %d: %.3f" % (mean_ppc, mode, r))
             assert r <= 1.0
         ctx.close()
+    # very high particles per cell (moments_seg.cuh: equal slices, one-pass raw sums, fp64 shift): ragged counts incl.
+    # empty and 1-3 particle cells, cells of up to ~40,000 particles, and a Mach-10 drift
+    for mean_ppc, seed, nx, ny, drift in ((600.0, 25, 16, 12, 0.0), (3000.0, 26, 8, 6, 0.0), (900.0, 27, 9, 5, 9.09)):
+        cfg, st = wl.ragged(nx=nx, ny=ny, seed=seed, mean_ppc=mean_ppc, drift=drift)
+        s, cs = _sorted_case(orc, cfg, st)
+        ctx = gpu.Context(cfg)
+        d = gpu.to_device(s)
+        for mode in (0, 1):
+            ref = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, mode)
+            mom = ctx.cell_moments(d["vx"], d["vy"], d["vz"], torch.from_numpy(cs).cuda(), mode)
+            r = moment_ratio(mom.cpu().numpy(), ref, absmom=abs_moments(s["vx"], s["vy"], s["vz"], cs, ref))
+            print("moments ppc %g (sliced) mode %d drift %g: %.3f" % (mean_ppc, mode, drift, r))
+            assert r <= 1.0
+        ctx.close()
     # all particles in one cell of a 4-cell grid (chunked accumulation path)
     rng = np.random.default_rng(4)
     n = 50_000
