@@ -21,7 +21,7 @@ static void fp_free_all(fp_ctx* c)
     cudaFree(c->hs_mom); cudaFree(c->hs_coef); cudaFree(c->hs_flags); cudaFree(c->hs_cell_start);
     if (c->hs_side) cudaStreamDestroy(c->hs_side);
     for (int k = 0; k < 4; ++k) if (c->hs_ev[k]) cudaEventDestroy(c->hs_ev[k]);
-    cudaFree(c->mlp.blob); cudaFree(c->mlp.tc_frags); cudaFree(c->mlp.wd_frags); cudaFree(c->mlp.w5_blob); cudaFree(c->mom_acc);
+    cudaFree(c->mlp.blob); cudaFree(c->mlp.tc_frags); cudaFree(c->mlp.wd_frags); cudaFree(c->mlp.w5_blob); cudaFree(c->mom_acc); cudaFree(c->upd_acc);
 }
 
 static void fp_timing_free(fp_ctx* c);

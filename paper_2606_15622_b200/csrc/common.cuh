@@ -60,6 +60,8 @@ struct fp_ctx {
     float    *cellc = nullptr;       // [ncell * 28] per-cell constants of the velocity update (update.cu)
     double   *mom_acc = nullptr;     // [ncell * 28] raw-sum accumulators of the high-ppc gather (moments_seg.cuh), lazy
     size_t    mom_acc_bytes = 0;
+    double   *upd_acc = nullptr;     // [ncell * 6] per-cell sums of the high-ppc update (update_seg.cuh), lazy
+    size_t    upd_acc_bytes = 0;
     // fp_step_host staging (allocated lazily)
     float    *hs_f[2][5] = {{nullptr}};
     uint32_t *hs_pid[2] = {nullptr, nullptr};

@@ -1,0 +1,147 @@
+// update_seg.cuh -- a6 at very high particles per cell (PAPER.md:282 30,000 particles per cell,
+// :491-497 500-1500).  Included by update.cu only.
+//
+// Same arithmetic as upd_giant_cell (pass A per 512-particle slice with all 32 lanes, per-slice sums combined in fp64,
+// fp64 epilogue, pass B as a streaming read-modify-write), but spread over the device: the particle index space is
+// cut into 512-particle slices regardless of cell boundaries, as in moments_seg.cuh.
+//   upd_seg_a_kernel: a warp stages its slice (vx, vy, vz, pid: four aligned bulk copies), runs pass A for every cell
+//     that intersects it (un-normalised c* over the velocities, six partial sums), adds the sums to the cell's fp64
+//     accumulators with atomics and writes the slice back with bulk stores;
+//   upd_seg_b_kernel: a warp walks the cells of its slice again, forms alpha / the recentring mean / the energy scale
+//     from the accumulators exactly as upd_giant_cell does, and rewrites its part of the cell.
+// 52 instead of 28 B per particle, every SM busy: 300 cells x 30,000 particles 1.55 ms -> see DESIGN.md.
+#pragma once
+
+#define UPD_SEG 512
+#define UPD_SEG_WARPS 4
+
+__device__ __forceinline__ int32_t upd_seg_first_cell(const int32_t* __restrict__ cell_start, int32_t ncell, int32_t a)
+{
+    int32_t lo = 0, hi = ncell;                                  // largest c with cell_start[c] <= a
+    while (hi - lo > 1) {
+        const int32_t mid = (lo + hi) >> 1;
+        if (cell_start[mid] <= a) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+__global__ void __launch_bounds__(UPD_SEG_WARPS * 32)
+upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
+                 const int32_t* __restrict__ cell_start, int64_t np, const float* __restrict__ cellc,
+                 double* __restrict__ acc, const __grid_constant__ upd_params Q)
+{
+    fpd_pdl();
+    __shared__ __align__(16) float stage[UPD_SEG_WARPS][4][UPD_SEG];
+    __shared__ __align__(8) uint64_t bars[UPD_SEG_WARPS];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* sx = stage[warp][0];
+    float* sy = stage[warp][1];
+    float* sz = stage[warp][2];
+    uint32_t* sp = reinterpret_cast<uint32_t*>(stage[warp][3]);
+    if (lane == 0) fpt_mbar_init(&bars[warp], 1);
+    __syncwarp();
+    const int64_t nslices = (np + UPD_SEG - 1) / UPD_SEG;
+    uint32_t phase = 0;
+    for (int64_t sl = (int64_t)blockIdx.x * UPD_SEG_WARPS + warp; sl < nslices; sl += (int64_t)gridDim.x * UPD_SEG_WARPS) {
+        const int32_t a = (int32_t)(sl * UPD_SEG), b = (int32_t)min((int64_t)a + UPD_SEG, np);
+        const int32_t nb = (b - a) & ~3;
+        fpt_fence_proxy_async();
+        __syncwarp();
+        if (lane == 0 && nb > 0) {
+            fpt_mbar_expect_tx(&bars[warp], 4u * (uint32_t)nb * 4u);
+            fpt_bulk_g2s(sx, vx + a, (uint32_t)nb * 4u, &bars[warp]);
+            fpt_bulk_g2s(sy, vy + a, (uint32_t)nb * 4u, &bars[warp]);
+            fpt_bulk_g2s(sz, vz + a, (uint32_t)nb * 4u, &bars[warp]);
+            fpt_bulk_g2s(sp, pid + a, (uint32_t)nb * 4u, &bars[warp]);
+        }
+        for (int32_t p = a + nb + lane; p < b; p += 32) { sx[p - a] = vx[p]; sy[p - a] = vy[p]; sz[p - a] = vz[p]; sp[p - a] = pid[p]; }
+        const int32_t c0 = upd_seg_first_cell(cell_start, Q.ncell, a);
+        if (nb > 0) { fpt_mbar_wait(&bars[warp], phase); phase ^= 1u; }
+        __syncwarp();
+        for (int32_t c = c0; c < Q.ncell; ++c) {
+            const int32_t cs0 = cell_start[c], cs1 = cell_start[c + 1];
+            if (cs0 >= b) break;
+            const int32_t s = max(cs0, a), e = min(cs1, b);
+            if (e <= s) continue;
+            float k[UPD_NC];
+            const float* cc = cellc + (size_t)c * UPD_NC;
+#pragma unroll
+            for (int q = 0; q < UPD_NC / 4; ++q) {
+                const float4 v = reinterpret_cast<const float4*>(cc)[q];
+                k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
+            }
+            if (k[23] == 0.0f) continue;                         // inactive cell: velocities stay
+            const upd_part pa = upd_pass_a<32>(sx, sy, sz, sp, s - a, e - s, lane, k, Q);
+            double D[6] = {(double)(pa.SNN.x + pa.SNN.y), (double)(pa.SCN.x + pa.SCN.y), (double)(pa.SM0.x + pa.SM0.y),
+                           (double)(pa.SM1.x + pa.SM1.y), (double)(pa.SM2.x + pa.SM2.y), (double)(pa.SQ.x + pa.SQ.y)};
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) {
+#pragma unroll
+                for (int q = 0; q < 6; ++q) D[q] += fpd_shfl_xor(D[q], d);
+            }
+            if (lane < 6) {
+                double mine = D[0];
+#pragma unroll
+                for (int q = 1; q < 6; ++q) if (lane == q) mine = D[q];
+                atomicAdd(&acc[(size_t)c * 6 + lane], mine);
+            }
+        }
+        // ---- c* back to global memory: aligned part by bulk stores, the ragged end of the last slice by plain stores
+        fpt_fence_proxy_async();
+        __syncwarp();
+        if (lane == 0 && nb > 0) {
+            fpt_bulk_s2g(vx + a, sx, (uint32_t)nb * 4u);
+            fpt_bulk_s2g(vy + a, sy, (uint32_t)nb * 4u);
+            fpt_bulk_s2g(vz + a, sz, (uint32_t)nb * 4u);
+            fpt_bulk_commit_wait();
+        }
+        for (int32_t p = a + nb + lane; p < b; p += 32) { vx[p] = sx[p - a]; vy[p] = sy[p - a]; vz[p] = sz[p - a]; }
+        __syncwarp();
+    }
+}
+
+__global__ void __launch_bounds__(UPD_SEG_WARPS * 32)
+upd_seg_b_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz,
+                 const int32_t* __restrict__ cell_start, int64_t np, const float* __restrict__ cellc,
+                 const double* __restrict__ acc, uint32_t* __restrict__ flags, const __grid_constant__ upd_params Q)
+{
+    fpd_pdl();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t nslices = (np + UPD_SEG - 1) / UPD_SEG;
+    for (int64_t sl = (int64_t)blockIdx.x * UPD_SEG_WARPS + warp; sl < nslices; sl += (int64_t)gridDim.x * UPD_SEG_WARPS) {
+        const int32_t a = (int32_t)(sl * UPD_SEG), b = (int32_t)min((int64_t)a + UPD_SEG, np);
+        const int32_t c0 = upd_seg_first_cell(cell_start, Q.ncell, a);
+        for (int32_t c = c0; c < Q.ncell; ++c) {
+            const int32_t cs0 = cell_start[c], cs1 = cell_start[c + 1];
+            if (cs0 >= b) break;
+            const int32_t s = max(cs0, a), e = min(cs1, b);
+            if (e <= s) continue;
+            float k[UPD_NC];
+            const float* cc = cellc + (size_t)c * UPD_NC;
+#pragma unroll
+            for (int q = 0; q < UPD_NC / 4; ++q) {
+                const float4 v = reinterpret_cast<const float4*>(cc)[q];
+                k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
+            }
+            if (k[23] == 0.0f) continue;
+            const double* D = acc + (size_t)c * 6;
+            const double invn = 1.0 / (double)(cs1 - cs0);
+            const double alpha2 = 1.0 + ((double)k[24] * D[0] + (double)k[25] * D[1]) * invn;
+            double alpha = 1.0;
+            if (!isfinite(alpha2) || alpha2 < 1e-6) { if (lane == 0 && cs0 >= a) flags[c] |= FP_FLAG_ALPHA; }   // once per cell
+            else alpha = sqrt(alpha2);
+            float mm0 = 0.f, mm1 = 0.f, mm2 = 0.f, scale = (float)(1.0 / alpha);
+            if (Q.conserve_mode == 1) {
+                const double m0 = D[2] * invn, m1 = D[3] * invn, m2 = D[4] * invn;
+                const double en = D[5] * invn - (m0 * m0 + m1 * m1 + m2 * m2);
+                mm0 = (float)m0; mm1 = (float)m1; mm2 = (float)m2;
+                if (en > 0.0 && isfinite(en)) scale = (float)sqrt((double)k[19] / en);
+            }
+            for (int32_t p = s + lane; p < e; p += 32) {
+                vx[p] = k[0] + fmaf(vx[p] - mm0, scale, k[3]);
+                vy[p] = k[1] + fmaf(vy[p] - mm1, scale, k[4]);
+                vz[p] = k[2] + fmaf(vz[p] - mm2, scale, k[5]);
+            }
+        }
+    }
+}

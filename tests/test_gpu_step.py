@@ -34,18 +34,20 @@ def _bits(a):
 
 
 # ------------------------------------------------------------------------------------------------ a6 update
-@pytest.mark.parametrize("case", ["couette-exact", "ragged-exact", "ragged-mlp", "ragged1d-exact"])
+@pytest.mark.parametrize("case", ["couette-exact", "ragged-exact", "ragged-mlp", "ragged1d-exact", "highppc-exact", "highppc-mlp"])
 @pytest.mark.parametrize("mode", [0, 1])
 def test_velocity_update(gpu, wl, orc, case, mode):
     import torch
     name, closure = case.split("-")
     cfg, st = {"couette": wl.couette, "ragged": wl.ragged,
-               "ragged1d": lambda: wl.ragged(nx=64, ny=1, seed=11, mean_ppc=150.0)}[name]()
+               "ragged1d": lambda: wl.ragged(nx=64, ny=1, seed=11, mean_ppc=150.0),
+               # few, huge cells (ragged: empty and 1-3 particle cells, cells of up to ~12,000): update_seg.cuh
+               "highppc": lambda: wl.ragged(nx=9, ny=7, seed=31, mean_ppc=900.0)}[name]()
     cfg = dict(cfg, conserve_mode=mode)
     s, cs, _ = orc.sort_by_cell(st, cfg)
     ncell = cs.shape[0] - 1
     rng = np.random.default_rng(17)
-    tau = rng.uniform(0.3, 2.0, size=ncell).astype(np.float32) if name == "ragged" else cfg["tau"]
+    tau = rng.uniform(0.3, 2.0, size=ncell).astype(np.float32) if name in ("ragged", "highppc") else cfg["tau"]
     if closure == "exact":
         mom = orc.cell_moments(s["vx"], s["vy"], s["vz"], cs, 1)
         coef, flags, _ = orc.closure_exact(mom, tau, cfg["eps2_scale"], cfg["min_count"])
