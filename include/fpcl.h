@@ -149,7 +149,7 @@ int fp_set_mlp_tensor_cores(fp_ctx* ctx, int32_t enable);
 
 /* Sampling outputs (they run once per sampled step, outside the per-step path).
  * fp_cell_diagnostics: 16 fp64 values per cell from the FULL record (PAPER.md:415 and Eq. 19-23 :632-657; the
- * normalisations are reading R8 of DESIGN.md): theta = P_kk/3; Delta_4 = <c^4> - 15 theta^2; Delta_4/(15 theta^2);
+ * normalisations are reading R10 of DESIGN.md): theta = P_kk/3; Delta_4 = <c^4> - 15 theta^2; Delta_4/(15 theta^2);
  * D_G = -1/2 log det(P/theta); D_q = |q_hat|^2/5 with q_hat = h/(2 theta^1.5); ds_eq = 3/2 log(theta/theta_inf) -
  * log(N/n_inf); ds_kin,G = ds_eq - (D_G - dg_inf); sigma_norm = |P - theta I|_F/theta; q_norm = |q_hat|;
  * m3_norm = |t|_F/theta^1.5; R_11, R_12, R_13, R_22, R_23, R_33, each <c_i c_j c^2>/(5 theta^2).  Empty or cold

@@ -303,7 +303,7 @@ void orc_closure_exact(int32_t ncell, const double *mom_full, const float *tau_c
  * Delta_4 = <(c_k c_k)^2> - 15 theta^2, theta = <c_k c_k>/3; Eq. 19-23 :632-657: Theta_ij = <c_i c_j>,
  * D_G = -1/2 log det(Theta/theta), ds_eq = 3/2 log(theta/theta_inf) - log(rho/rho_inf),
  * ds_kin,G = ds_eq - (D_G - D_G,inf), D_q = |q_hat|^2 / 5 with q_hat = <c |c|^2> / (2 theta^(3/2))).
- * "norm" = divided by the local Maxwellian scale (reading R8: the paper only says
+ * "norm" = divided by the local Maxwellian scale (reading R10: the paper only says
  * "nondimensionalization by the corresponding local Maxwellian scales"): Delta_4 / (15 theta^2),
  * R_ij / (5 theta^2) (a Maxwellian has <c_i c_j c^2> = 5 theta^2 delta_ij), sigma_norm = |P - theta I|_F / theta,
  * q_norm = |q_hat|, m3_norm = |t|_F / theta^(3/2) (all 27 index triples).  DM6 = <(c^2)^3> needs a sixth-order
@@ -352,7 +352,7 @@ void orc_cell_diagnostics(int32_t ncell, const double *mom_full, double theta_in
 
 /* DM6 = <(c_k c_k)^3>, the sixth central moment of PAPER.md:415, per cell from the cell-sorted particles (the FULL
  * record stops at fifth order).  dm6[cell] = (1/N) sum (|v - U|^2)^3 with U the cell mean (recomputed here); empty
- * cell: 0.  A Maxwellian has <c^6> = 105 theta^3, which is the "local Maxwellian scale" of DM6_norm (reading R8). */
+ * cell: 0.  A Maxwellian has <c^6> = 105 theta^3, which is the "local Maxwellian scale" of DM6_norm (reading R10). */
 void orc_cell_dm6(const float *vx, const float *vy, const float *vz, const int32_t *cell_start, int32_t ncell, double *dm6)
 {
     for (int32_t cell = 0; cell < ncell; ++cell) {

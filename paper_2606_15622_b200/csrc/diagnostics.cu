@@ -1,6 +1,6 @@
 // diagnostics.cu -- NEXT-2: sampling outputs of the closure path.
 //   fp_cell_diagnostics: per-cell nonequilibrium diagnostics from the FULL moment record (PAPER.md:415 R_ij, Delta_4,
-//     theta; Eq. 19-23 :632-657 D_G, ds_eq, ds_kin,G, D_q; normalisations: DESIGN.md R8).
+//     theta; Eq. 19-23 :632-657 D_G, ds_eq, ds_kin,G, D_q; normalisations: DESIGN.md R10).
 //   fp_cell_sixth_moment: the sixth central moment DM6 = <(c^2)^3>, which the FULL record does not carry.
 //   fp_average_results: running time average of sampled per-cell fields.
 // Both are one thread per value, fp64, HBM-bound by construction (232 B read + 128 B written per cell; 16 B read +
