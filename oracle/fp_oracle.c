@@ -18,8 +18,11 @@
  * brute-force Cramer, axis-permutation and scaling symmetries, Table 1 entries as printed; MLP -- hand cases,
  * parameter counts, independent numpy forward; Philox -- Random123 known-answer vectors and
  * numpy's Philox bit generator; update -- Eq. 15 identity, noise-off Langevin decay, conservation, OU
- * stationarity; walls -- half-range Maxwellian moments; diagnostics -- hand values on octahedral ensembles, numpy
- * slogdet, rotation invariance, Maxwellian limits.
+ * stationarity, the drift N_i recovered from the OUTPUT velocities against Eq. 14 typed out in numpy and against
+ * the relaxation identities the exact closure imposes (<N_i c_j + N_j c_i> = 0, <N_i c^2 + 2 c_i c.N> = 5 h_i/(3 tau)),
+ * an N = 2 cell is updated; walls -- half-range Maxwellian moments on the lid (y-wall) and on both Couette plates
+ * (x-walls, distinct tangential wall speeds); diagnostics -- hand values on octahedral ensembles, numpy
+ * slogdet, rotation invariance, Maxwellian limits, N = 3 cells whose determinant rounds positive.
  * Parity unpinned (no independent source exists): the value of eps^2 (R2-e), the low-count /
  * singular-cell policy (R3-c), the 16-feature definitions (R4), and the wall re-emission details (R7) as
  * compared with the paper's own runs.

@@ -148,3 +148,23 @@ def test_dm6_hand_and_maxwellian(orc):
     got = orc.cell_dm6(g[:, 0], g[:, 1], g[:, 2], np.array([0, 0, n], dtype=np.int32))
     assert got[0] == 0.0                                            # empty cell
     assert got[1] == pytest.approx(105 * 0.5 ** 3, rel=0.03)        # relative sd of the estimate ~ 10 / sqrt(n)
+
+
+def test_three_particle_cell_is_defined_singular(orc):
+    """Reading R10: a cell with N < 4 has a covariance of rank <= N - 1, so D_G = +inf and ds_kin,G = -inf whatever the
+    rounding of its (mathematically zero) determinant says; N = 4 in general position is regular.  theta > 0 in both."""
+    # three-particle sets whose rank-2 covariance has a determinant that ROUNDS to a small positive number in fp64
+    # (found by search): without the N < 4 rule they would report a finite D_G ~ 19
+    for v3 in ([[0.1, -0.1, 0.4], [0.1, -0.3, 0.2], [0.8, 0.6, -0.4]],
+               [[-0.6, -0.3, 0.1], [-0.6, -0.1, -0.1], [0.3, 0.1, 0.2]],
+               [[0.3, -0.2, 0.5], [-0.4, 0.6, 0.1], [0.2, 0.1, -0.7]]):
+        d3, m3 = _diag_of(orc, np.float32(v3))
+        assert m3[0] == 3 and d3["theta"] > 0.05
+        assert d3["DG"] == np.inf and d3["dskin"] == -np.inf
+        assert np.isfinite(d3["d4"]) and np.isfinite(d3["sig"]) and np.isfinite(d3["dseq"])
+    v4 = np.float32([[0.3, -0.2, 0.5], [-0.4, 0.6, 0.1], [0.2, 0.1, -0.7], [-0.1, -0.5, 0.1]])
+    d4, m4 = _diag_of(orc, v4)
+    c = v4.astype(np.float64) - v4.astype(np.float64).mean(0)
+    Th = c.T @ c / 4
+    sign, logdet = np.linalg.slogdet(Th / (np.trace(Th) / 3))
+    assert sign > 0 and d4["DG"] == pytest.approx(-0.5 * logdet, rel=1e-10)

@@ -171,3 +171,145 @@ def test_periodic_and_body(orc):
     assert np.all(r >= 2.0) and np.all(r < 2.0 * 1.00001)                         # pushed out to the surface
     vr = (out["vx"][2:] * (out["x"][2:] - 4) + out["vy"][2:] * (out["y"][2:] - 4)) / r
     assert np.all(vr > 0)                                                          # re-emitted outwards
+
+
+# ------------------------------------------------------------------------------------------------ Eq. 14 pins
+def _recover_N(orc, v, cs, pid, mom, coef, tau, cfg, step, alpha):
+    """N_i per particle from the oracle's OUTPUT of a conserve_mode-0 update, by inverting Eq. 13:
+    N = (alpha c* - c E1 - sqrt(theta (1 - E2)) xi) / ((1 - E1) tau), with the separately pinned normals."""
+    vx, vy, vz, fl = orc.velocity_update(v[:, 0], v[:, 1], v[:, 2], pid, cs, mom, coef[None, :], np.float32(tau), cfg, step)
+    assert fl[0] == 0
+    U, theta = mom[0, 1:4], (mom[0, 4] + mom[0, 7] + mom[0, 9]) / 3
+    tau32 = float(np.float32(tau))
+    a = cfg["dt"] / tau32
+    E1, E2 = math.exp(-a), math.exp(-2 * a)
+    xi = orc.normals(pid, step, 0, cfg["seed"])
+    cstar = np.stack([vx, vy, vz], 1).astype(np.float64) - U
+    c = v.astype(np.float64) - U
+    w = c * E1 + math.sqrt(theta * (1 - E2)) * xi
+    kap = (1 - E1) * tau32
+    if alpha is None:
+        return cstar, w, kap, c, theta, (E1, E2, tau32)
+    return (alpha * cstar - w) / kap, c, theta, (E1, E2, tau32)
+
+
+def _eq14_numpy(c, theta, P, h, coef, tau, eps2_scale):
+    """Eq. 14 typed out: N_i = (C_ij + delta_ij/tau) c_j + gam_i (c^2 - 3 theta) - eps2 (c_i c^2 - h_i),
+    C symmetric from (c11, c12, c13, c22, c23, c33), eps2 = eps2_scale |det(P - theta I)| / (tau theta^4) (R2-e)."""
+    C = np.array([[coef[0], coef[1], coef[2]], [coef[1], coef[3], coef[4]], [coef[2], coef[4], coef[5]]], dtype=np.float64)
+    gam = np.asarray(coef[6:9], dtype=np.float64)
+    Pm = np.array([[P[0], P[1], P[2]], [P[1], P[3], P[4]], [P[2], P[4], P[5]]])
+    eps2 = eps2_scale * abs(np.linalg.det(Pm - theta * np.eye(3))) / (tau * theta ** 4)
+    c2 = (c ** 2).sum(1)
+    return c @ (C + np.eye(3) / tau).T + gam[None, :] * (c2 - 3 * theta)[:, None] - eps2 * (c * c2[:, None] - h[None, :])
+
+
+@pytest.mark.parametrize("eps2_scale", [1.0, 5.0])
+def test_update_drift_matches_eq14(orc, eps2_scale):
+    """The non-Langevin drift inside the update, per particle, against Eq. 14 written out in numpy: nine distinct
+    coefficients (no accidental symmetry), theta != 1 (so a lost 1/theta^4 shows), eps2 > 0."""
+    cfg, v, cs, pid = _cell(orc, 400, 21)
+    v = (v * np.float32(1.3)).astype(np.float32)                          # theta ~ 0.85
+    cfg.update(conserve_mode=0, eps2_scale=float(np.float32(eps2_scale)), dt=float(np.float32(0.2)), seed=13)
+    tau = 0.8
+    mom = orc.cell_moments(v[:, 0], v[:, 1], v[:, 2], cs, 1)
+    coef = np.float32([-1.1, 0.23, -0.31, -0.87, 0.12, -1.4, 0.07, -0.05, 0.11]) / np.float32(tau)
+    U, P = mom[0, 1:4], mom[0, 4:10]
+    theta = (P[0] + P[3] + P[5]) / 3
+    t = mom[0, 10:20]                                                     # 111,112,113,122,123,133,222,223,233,333
+    h = np.array([t[0] + t[3] + t[5], t[1] + t[6] + t[8], t[2] + t[7] + t[9]])
+    c = v.astype(np.float64) - U
+    tau32 = float(np.float32(tau))
+    N_ref = _eq14_numpy(c, theta, P, h, coef.astype(np.float64), tau32, cfg["eps2_scale"])
+    assert np.abs(N_ref - c @ (np.diag([1 / tau32] * 3) + np.diag(coef[[0, 3, 5]].astype(np.float64))).T).max() > 0.05
+    a = cfg["dt"] / tau32
+    E1, E2 = math.exp(-a), math.exp(-2 * a)
+    alpha2 = 1 + tau32 / (3 * theta) * (tau32 * (1 - E1) ** 2 * (N_ref ** 2).sum(1).mean()
+                                        + 2 * (E1 - E2) * (c * N_ref).sum(1).mean())          # Eq. 15 (:178)
+    N_got, _, _, _ = _recover_N(orc, v, cs, pid, mom, coef, tau, cfg, 7, math.sqrt(alpha2))
+    # output velocities are fp32: |dN| <~ 6e-8 |v| alpha / ((1 - E1) tau)
+    np.testing.assert_allclose(N_got, N_ref, atol=3e-7 * np.abs(v).max() / ((1 - E1) * tau32))
+    assert abs(N_got.mean(0)).max() < 1e-6                                # <N_i> = 0 for any coefficients
+
+
+def test_update_drift_satisfies_closure_constraints(orc):
+    """Independent of any retyped Eq. 14: with the EXACT closure's coefficients the drift the update applies must
+    reproduce the relaxation rates the closure imposes (Eq. 3 :69, :124; oracle header):
+      <N_i c_j + N_j c_i> = <A_i c_j + A_j c_i> + 2 P_ij / tau = 0                     (stress rate 2/tau)
+      <N_i c^2 + 2 c_i c.N> = -(4/(3 tau)) h_i + 3 h_i / tau = (5/(3 tau)) h_i         (heat-flux rate 4/(3 tau))
+    where A = N - c/tau is the drift of Eq. 8 and the diffusion terms (2 theta/tau delta_ij; <c_i> = 0) are moved to
+    the right.  alpha is not assumed: it is fixed by the trace of the first identity, <c.N> = 0, and must then satisfy
+    Eq. 15 with the recovered N."""
+    cfg, st, _ = wl.grad13_cells(1, 1, 3000, seed=31, smax=0.25, qmax=0.15)
+    v = (np.stack([st["vx"], st["vy"], st["vz"]], 1) * np.float32(1.2) + np.float32([0.4, -0.1, 0.2])).astype(np.float32)
+    cs = np.array([0, v.shape[0]], dtype=np.int32)
+    pid = st["pid"]
+    tau = 0.9
+    cfg.update(conserve_mode=0, eps2_scale=float(np.float32(2.0)), dt=float(np.float32(0.25)), seed=4)
+    mom = orc.cell_moments(v[:, 0], v[:, 1], v[:, 2], cs, 1)
+    coef, flags, kappa = orc.closure_exact(mom, float(np.float32(tau)), cfg["eps2_scale"])
+    assert flags[0] == 0 and kappa[0] < 1e4
+    coef32 = coef[0].astype(np.float32)
+    cstar, w, kap, c, theta, (E1, E2, tau32) = _recover_N(orc, v, cs, pid, mom, coef32, tau, cfg, 3, None)
+    alpha = (c * w).sum(1).mean() / (c * cstar).sum(1).mean()             # from <c.N> = 0
+    N = (alpha * cstar - w) / kap
+    alpha2_eq15 = 1 + tau32 / (3 * theta) * (tau32 * (1 - E1) ** 2 * (N ** 2).sum(1).mean() + 2 * (E1 - E2) * (c * N).sum(1).mean())
+    assert abs(alpha * alpha - alpha2_eq15) < 1e-5                         # fp32 coefficients and velocities
+    assert alpha > 1.0                                                     # Eq. 15 with <c.N> = 0: alpha^2 = 1 + (...) <N.N>
+    S = np.einsum("pi,pj->ij", N, c) / c.shape[0]
+    S = S + S.T
+    scale = theta / tau32
+    assert np.abs(S).max() < 2e-5 * scale, S / scale                       # all six stress identities
+    t = mom[0, 10:20]
+    h = np.array([t[0] + t[3] + t[5], t[1] + t[6] + t[8], t[2] + t[7] + t[9]])
+    c2 = (c ** 2).sum(1)
+    H = (N * c2[:, None] + 2 * c * (c * N).sum(1)[:, None]).mean(0)
+    np.testing.assert_allclose(H, 5.0 / (3.0 * tau32) * h, atol=2e-4 * theta ** 1.5 / tau32)
+    assert np.abs(h).max() > 0.01 * theta ** 1.5                           # the heat flux is not trivially zero
+
+
+def test_two_particle_cell_is_updated(orc):
+    """R5: a cell with N = 2 and theta > 0 is updated (only N < 2 or theta <= 0 is skipped): conserve_mode 1 keeps its
+    momentum and energy and the velocities change."""
+    v = np.float32([[0.3, -0.2, 0.5], [-0.4, 0.6, 0.1], [9, 9, 9]])
+    cs = np.array([0, 2, 3], dtype=np.int32)
+    cfg, _ = wl.couette()
+    cfg.update(conserve_mode=1, seed=2, dt=float(np.float32(0.3)))
+    mom = orc.cell_moments(v[:, 0], v[:, 1], v[:, 2], cs, 0)
+    vx, vy, vz, fl = orc.velocity_update(v[:, 0], v[:, 1], v[:, 2], np.arange(3, dtype=np.uint32), cs, mom,
+                                         np.tile(LANG(1.0), (2, 1)), 1.0, cfg, 0)
+    new = np.stack([vx, vy, vz], 1).astype(np.float64)
+    assert fl.tolist() == [0, orc.FLAG_SKIPPED]
+    assert np.array_equal(new[2], v[2]) and np.abs(new[:2] - v[:2]).max() > 0.01
+    old = v[:2].astype(np.float64)
+    np.testing.assert_allclose(new[:2].mean(0), old.mean(0), atol=2e-7)
+    np.testing.assert_allclose(((new[:2] - new[:2].mean(0)) ** 2).sum(), ((old - old.mean(0)) ** 2).sum(), rtol=1e-6)
+
+
+# ------------------------------------------------------------------------------------------------ S7: x-walls
+@pytest.mark.parametrize("side", [0, 1])
+def test_couette_plate_reemission(orc, side):
+    """BASELINE config 1 geometry: diffuse plates at xmin/xmax moving in y (and, to tell the
+    tangential components apart, a different speed in z).  Every particle crosses the plate: v_x must point into the
+    gas with the half-range law, <v_y> = U_w,y, <v_z> = U_w,z, tangential variances theta_w."""
+    n, th_w = 200_000, 0.6
+    uwy, uwz = (-0.3, 0.11) if side == 0 else (0.3, -0.17)
+    walls = [(1, th_w, 0, -0.3, 0.11), (1, th_w, 0, 0.3, -0.17), (0, 0.5, 0, 0, 0), (0, 0.5, 0, 0, 0)]
+    cfg = wl.make_config(8, 1, 0.125, 1.0, 1.0, 1.0, walls, seed=17)
+    rng = np.random.default_rng(1)
+    x0 = 0.1 if side == 0 else 0.9
+    st = dict(x=np.full(n, x0, np.float32), y=rng.uniform(0.1, 0.9, n).astype(np.float32),
+              vx=np.full(n, -0.5 if side == 0 else 0.5, np.float32), vy=np.full(n, 7.0, np.float32) * 0,
+              vz=np.full(n, 3.0, np.float32), pid=np.arange(n, dtype=np.uint32))
+    out = orc.stream_walls(st, cfg, step=2)
+    vn = out["vx"].astype(np.float64) * (1.0 if side == 0 else -1.0)       # into the gas
+    se = 5 / math.sqrt(n)
+    assert np.all(vn > 0)
+    assert abs(vn.mean() - math.sqrt(math.pi * th_w / 2)) < se * math.sqrt(th_w)
+    assert abs((vn ** 2).mean() - 2 * th_w) < se * 2 * th_w
+    assert abs(out["vy"].mean() - uwy) < se * math.sqrt(th_w) and abs(out["vz"].mean() - uwz) < se * math.sqrt(th_w)
+    assert abs(out["vy"].var() - th_w) < se * 2 * th_w and abs(out["vz"].var() - th_w) < se * 2 * th_w
+    xw = np.float32(0.0 if side == 0 else 1.0)
+    xe = np.float32(x0) + np.float32(-0.5 if side == 0 else 0.5)            # exact in fp32
+    np.testing.assert_array_equal(out["x"], xw + (xw - xe))
+    assert np.array_equal(out["y"], st["y"])                                # vy = 0: y untouched, ny = 1
