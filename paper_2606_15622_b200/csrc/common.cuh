@@ -62,6 +62,7 @@ struct fp_ctx {
     size_t    mom_acc_bytes = 0;
     double   *upd_acc = nullptr;     // [ncell * 6] per-cell sums of the high-ppc update (update_seg.cuh), lazy
     size_t    upd_acc_bytes = 0;
+    bool      upd_attr[4] = {false, false, false, false};   // shared-memory attribute set for update_warp_kernel<4|8|16|32> (per context, i.e. per device)
     // fp_step_host staging (allocated lazily)
     float    *hs_f[2][5] = {{nullptr}};
     uint32_t *hs_pid[2] = {nullptr, nullptr};
