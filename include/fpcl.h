@@ -10,9 +10,19 @@
  *    gives a human-readable string for the last failure on that context.
  *  - Pointers are DEVICE pointers unless the name starts with h_ (host).  The caller owns every particle, grid,
  *    coefficient and weight buffer; the library never allocates or frees them.  The library owns only fp_ctx and
- *    the scratch sized at fp_create (sort ping-pong buffers, digit histograms, uploaded MLP parameters).
+ *    its scratch.  Everything whose size follows from fp_params is allocated by fp_create (sort ping-pong buffers,
+ *    digit histograms, per-cell update constants, the accumulators of the high-particles-per-cell paths).  Two
+ *    pieces depend on later arguments and are allocated on FIRST USE unless fp_reserve was called: the packed
+ *    parameters of a surrogate network (sized by its shape; a differently shaped network re-allocates) and the
+ *    device staging buffers of fp_step_host.  A first-use allocation is a cudaMalloc and may stall the stream.
  *  - All calls are asynchronous on the caller's stream (a cudaStream_t passed as void*; NULL = legacy default
- *    stream) and never synchronise the host.
+ *    stream) and, apart from the first-use allocations above, fp_step_host, fp_timing_read and fp_check, never
+ *    synchronise the host.
+ *  - cell_start must be a monotone prefix sum over the cells with cell_start[0] >= 0 and cell_start[ncell] == np
+ *    (what fp_sort_by_cell writes).  fp_cell_moments and fp_velocity_update verify this ON THE DEVICE while they read it:
+ *    cells with bad boundaries are skipped (no out-of-range access) and a sticky state word is set in the context;
+ *    because the calls are asynchronous the failing call itself returns FP_OK and every LATER entry point on the
+ *    context returns FP_ERR_STATE until fp_check (which synchronises) has reported and cleared it.
  *  - Numerical trouble in a cell is NOT an error code: it sets FP_FLAG_* bits in flags[cell] and the cell gets the
  *    documented fallback (readings R3-c, R5).
  *  - Particle arrays are SoA fp32: x, y, vx, vy, vz [np] and a persistent particle id pid [np] (uint32) that
@@ -36,7 +46,7 @@ extern "C" {
 /* error codes */
 #define FP_OK               0
 #define FP_ERR_ARG         (-1)   /* null / misaligned pointer, size mismatch, bad enum                  */
-#define FP_ERR_STATE       (-2)   /* call sequence violated (e.g. np > max_particles)                     */
+#define FP_ERR_STATE       (-2)   /* np > max_particles; cell_start not a sorted prefix (see Conventions)   */
 #define FP_ERR_CUDA        (-3)   /* a CUDA runtime call failed; see fp_last_error                        */
 #define FP_ERR_UNSUPPORTED (-4)   /* e.g. an MLP wider than the fused kernel supports                     */
 
@@ -107,6 +117,14 @@ const char* fp_last_error(const fp_ctx* ctx);
 /* Library version / build string (static storage). */
 const char* fp_version(void);
 
+/* Allocate now what would otherwise be allocated on first use (Conventions): the packed-parameter scratch for a
+ * network of h_mlp's shape (h_mlp nullable: skip) and, if host_staging != 0, the device buffers of fp_step_host
+ * (6 arrays of max_particles + per-cell outputs, twice).  Synchronous (cudaMalloc).  After it no call on the context
+ * allocates, unless a network of another shape is passed. */
+int fp_reserve(fp_ctx* ctx, const fp_mlp* h_mlp /* nullable */, int32_t host_staging);
+/* Synchronise `stream`, report (FP_ERR_STATE) and clear the sticky device-side state word; FP_OK if it was clear. */
+int fp_check(fp_ctx* ctx, void* stream);
+
 /* a2 -- cell index + stable sort (R1).  key = iy*nx + ix with
  * ix = clamp(floorf((x - x0) * (1/dx)), 0, nx-1) in fp32.  Writes the permuted SoA into the *_out arrays (which
  * may not alias the inputs), cell_start[ncell+1] (cell_start[k] = #particles with key < k) and, if non-null,
@@ -125,7 +143,8 @@ int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, c
 /* a4 -- exact cubic-FP closure: assemble and solve the 9x9 moment-matching system per cell (Eq. 10
  * :121, Table 1 :130-136; derivation DESIGN.md R2, scaling and flags R3).  tau_cell nullable (then params.tau).
  * coef [ncell*9] fp32, flags [ncell] (overwritten).  kappa_est nullable: if given receives the
- * library's estimate (a lower bound) of the condition number of the scaled system, the same number that
+ * library's estimate (a LOWER BOUND, typically within a factor ~30 of kappa_1; tests/test_gpu_parity.py states the
+ * measured factor) of the condition number of the scaled system, the same number that
  * decides FP_FLAG_ILLCOND (>= 1e8): max(||A||_inf ||y||_inf / ||b||_inf, max|pivot| / min|pivot|). */
 int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell /* nullable */,
                      float* coef, uint32_t* flags, double* kappa_est /* nullable */, void* stream);
@@ -192,9 +211,10 @@ int fp_step(fp_ctx* ctx, int64_t np,
 
 /* Host-buffer convenience used by the end-to-end measurement: uploads the six SoA arrays from host memory
  * (pinned or pageable), runs fp_step on internally held device buffers sized max_particles, and downloads the
- * updated SoA plus cell_start, flags and coef back into the host arrays.  The upload of vz (needed only by the
- * payload gather) and the download of x, y, pid (final after the gather) run on a context-owned side stream so that
- * they overlap the kernels; both streams are synchronised before returning.
+ * updated SoA plus cell_start, flags and coef back into the host arrays.  All uploads run on the caller's stream
+ * before the first kernel (the stream kernel rewrites vx, vy, vz of re-emitted particles, so none may still be in
+ * flight); the download of x, y, pid (final after the gather) runs on a context-owned side stream and overlaps the
+ * moment, closure and update kernels; both streams are synchronised before returning.
  * h_* are HOST pointers; h_coef [ncell*9], h_flags [ncell], h_cell_start [ncell+1]. */
 int fp_step_host(fp_ctx* ctx, int64_t np,
                  float* h_x, float* h_y, float* h_vx, float* h_vy, float* h_vz, uint32_t* h_pid,

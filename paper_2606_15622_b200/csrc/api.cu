@@ -17,6 +17,8 @@ static void fp_free_all(fp_ctx* c)
 {
     cudaFree(c->key_a); cudaFree(c->key_b); cudaFree(c->idx_a); cudaFree(c->idx_b);
     cudaFree(c->block_hist); cudaFree(c->bin_total); cudaFree(c->cellc);
+    if (c->h_err) cudaFreeHost(c->h_err);
+    cudaFree(c->d_errdev);
     for (int s = 0; s < 2; ++s) { for (int k = 0; k < 5; ++k) cudaFree(c->hs_f[s][k]); cudaFree(c->hs_pid[s]); }
     cudaFree(c->hs_mom); cudaFree(c->hs_coef); cudaFree(c->hs_flags); cudaFree(c->hs_cell_start);
     if (c->hs_side) cudaStreamDestroy(c->hs_side);
@@ -42,6 +44,8 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
     c->p = q;
     { const char* e = getenv("FPCL_MLP_FP32"); c->mlp_force_fp32 = e && e[0] == '1'; }
     { const char* e = getenv("FPCL_SORT_UNPACKED"); c->sort_no_pack = e && e[0] == '1'; }
+    c->env_mom_seg = getenv("FPCL_MOM_SEG") != nullptr; c->env_mom_no_seg = getenv("FPCL_MOM_NO_SEG") != nullptr;
+    c->env_upd_seg = getenv("FPCL_UPD_SEG") != nullptr; c->env_upd_no_seg = getenv("FPCL_UPD_NO_SEG") != nullptr;
     c->ncell = q.nx * q.ny;
     int bits = 0;
     while (((int64_t)1 << bits) < (int64_t)c->ncell) ++bits;
@@ -66,7 +70,13 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
               cudaMalloc((void**)&c->block_hist, 2 * c->block_hist_elems * 4) == cudaSuccess &&
               cudaMemset(c->block_hist, 0, 2 * c->block_hist_elems * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->bin_total, 512 * 4) == cudaSuccess &&
-              cudaMalloc((void**)&c->cellc, (size_t)c->ncell * 28 * 4) == cudaSuccess;
+              cudaMalloc((void**)&c->cellc, (size_t)c->ncell * 28 * 4) == cudaSuccess &&
+              cudaMalloc((void**)&c->mom_acc, (size_t)c->ncell * 28 * sizeof(double)) == cudaSuccess &&
+              cudaMalloc((void**)&c->upd_acc, (size_t)c->ncell * 6 * sizeof(double)) == cudaSuccess &&
+              cudaHostAlloc((void**)&c->h_err, sizeof(uint32_t), cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostGetDevicePointer((void**)&c->d_err, c->h_err, 0) == cudaSuccess &&
+              cudaMalloc((void**)&c->d_errdev, 4) == cudaSuccess && cudaMemset(c->d_errdev, 0, 4) == cudaSuccess;
+    if (ok) *c->h_err = 0;
     if (!ok) { fp_free_all(c); delete c; cudaGetLastError(); return FP_ERR_CUDA; }
     *out = c;
     return FP_OK;
@@ -115,6 +125,7 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
     if (closure == 1 && !h_mlp) return fp_fail(ctx, FP_ERR_ARG, "fp_step: surrogate closure needs h_mlp");
     if (tau_mode == 1 && !tau_cell) return fp_fail(ctx, FP_ERR_ARG, "fp_step: tau_mode 1 needs tau_cell");
     if (np > ctx->p.max_particles) return fp_fail(ctx, FP_ERR_STATE, "fp_step: np > max_particles");
+    if (fp_state_check(ctx, "fp_step") != FP_OK) return FP_ERR_STATE;
     if (np > 0 && (!x_a || !y_a || !vx_a || !vy_a || !vz_a || !pid_a || !x_b || !y_b || !vx_b || !vy_b || !vz_b || !pid_b))
         return fp_fail(ctx, FP_ERR_ARG, "fp_step: null particle pointer");
     cudaStream_t st = (cudaStream_t)stream;
@@ -209,6 +220,30 @@ static int fp_host_stage_alloc(fp_ctx* c)
     return FP_OK;
 }
 
+int fpi_mlp_reserve(fp_ctx* ctx, const fp_mlp* h_mlp);
+
+extern "C" int fp_reserve(fp_ctx* ctx, const fp_mlp* h_mlp, int32_t host_staging)
+{
+    if (!ctx) return FP_ERR_ARG;
+    int rc = FP_OK;
+    if (h_mlp && (rc = fpi_mlp_reserve(ctx, h_mlp)) != FP_OK) return rc;
+    if (host_staging && (rc = fp_host_stage_alloc(ctx)) != FP_OK) return rc;
+    return FP_OK;
+}
+
+extern "C" int fp_check(fp_ctx* ctx, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    FP_CUDA_OK(ctx, cudaStreamSynchronize((cudaStream_t)stream));
+    const uint32_t e = *(volatile uint32_t*)ctx->h_err;
+    *(volatile uint32_t*)ctx->h_err = 0;
+    FP_CUDA_OK(ctx, cudaMemset(ctx->d_errdev, 0, 4));
+    if (e & FP_DEVERR_CELL_START)
+        return fp_fail(ctx, FP_ERR_STATE, "fp_check: cell_start was not a monotone prefix sum ending at np in an earlier call; "
+                                          "the cells concerned were skipped");
+    return FP_OK;
+}
+
 extern "C" int fp_step_host(fp_ctx* ctx, int64_t np,
                             float* h_x, float* h_y, float* h_vx, float* h_vy, float* h_vz, uint32_t* h_pid,
                             int32_t closure, const fp_mlp* h_mlp, float relax_w, uint64_t step,
@@ -217,21 +252,17 @@ extern "C" int fp_step_host(fp_ctx* ctx, int64_t np,
     if (!ctx) return FP_ERR_ARG;
     if (np < 0 || np > ctx->p.max_particles) return fp_fail(ctx, FP_ERR_STATE, "fp_step_host: np out of range");
     if (np > 0 && (!h_x || !h_y || !h_vx || !h_vy || !h_vz || !h_pid)) return fp_fail(ctx, FP_ERR_ARG, "fp_step_host: null host pointer");
-    int rc = fp_host_stage_alloc(ctx);
+    int rc = fp_host_stage_alloc(ctx);                // no-op after fp_reserve(ctx, ..., 1) or the first call
     if (rc != FP_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     float* hp[5] = {h_x, h_y, h_vx, h_vy, h_vz};
     const size_t nb = (size_t)np * 4;
     cudaStream_t side = ctx->hs_side;
-    // host -> device: x, y, vx, vy, pid feed the stream kernel and the key sort; vz is needed only by the payload
-    // gather, so it travels on the side stream while those kernels run
-    FP_CUDA_OK(ctx, cudaEventRecord(ctx->hs_ev[0], st));                 // everything the caller queued before us
-    for (int k = 0; k < 4; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_f[0][k], hp[k], nb, cudaMemcpyHostToDevice, st));
+    // host -> device, all on the caller's stream: the stream kernel reads x, y, vx, vy, pid and REWRITES vx, vy, vz of
+    // every particle it re-emits at a wall or the body, so no input may still be in flight when it starts
+    for (int k = 0; k < 5; ++k) if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_f[0][k], hp[k], nb, cudaMemcpyHostToDevice, st));
     if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_pid[0], h_pid, nb, cudaMemcpyHostToDevice, st));
-    FP_CUDA_OK(ctx, cudaStreamWaitEvent(side, ctx->hs_ev[0], 0));
-    if (nb) FP_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hs_f[0][4], hp[4], nb, cudaMemcpyHostToDevice, side));
-    FP_CUDA_OK(ctx, cudaEventRecord(ctx->hs_ev[1], side));
-    ctx->ev_before_gather = ctx->hs_ev[1];
+    ctx->ev_before_gather = nullptr;
     ctx->ev_after_gather = ctx->hs_ev[2];
     rc = fp_step(ctx, np, ctx->hs_f[0][0], ctx->hs_f[0][1], ctx->hs_f[0][2], ctx->hs_f[0][3], ctx->hs_f[0][4], ctx->hs_pid[0],
                  ctx->hs_f[1][0], ctx->hs_f[1][1], ctx->hs_f[1][2], ctx->hs_f[1][3], ctx->hs_f[1][4], ctx->hs_pid[1],

@@ -192,6 +192,43 @@ extern "C" int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride
     return fpi_closure_mlp(ctx, mom, mom_stride, tau_cell, h_mlp, relax_w, coef, flags, false, (cudaStream_t)stream);
 }
 
+// Size every packed-parameter buffer a network of this shape can need (whichever kernel is selected later), now.
+// fp_closure_mlp grows the same buffers on first use otherwise; see fp_reserve in include/fpcl.h.
+int fpi_mlp_reserve(fp_ctx* ctx, const fp_mlp* h_mlp)
+{
+    if (!h_mlp || !h_mlp->h_dims || h_mlp->n_layers < 1 || h_mlp->n_layers > FPCL_MAX_LAYERS)
+        return fp_fail(ctx, FP_ERR_ARG, "fp_reserve: bad fp_mlp description");
+    const fp_mlp& M = *h_mlp;
+    fp_mlp_dev& C = ctx->mlp;
+    int off = 0;
+    for (int l = 0; l <= M.n_layers; ++l)
+        if (M.h_dims[l] < 1 || M.h_dims[l] > 1024) return fp_fail(ctx, FP_ERR_UNSUPPORTED, "fp_reserve: layer width must be in [1,1024]");
+    for (int l = 0; l < M.n_layers; ++l) off += M.h_dims[l] * pad8(M.h_dims[l + 1]) + pad8(M.h_dims[l + 1]);
+    off += 2 * pad8(M.h_dims[0]) + 32;
+    auto ensure = [&](void** ptr, size_t* have, size_t need) -> int {
+        if (*have >= need) return FP_OK;
+        if (*ptr) FP_CUDA_OK(ctx, cudaFree(*ptr));
+        *ptr = nullptr; *have = 0;
+        FP_CUDA_OK(ctx, cudaMalloc(ptr, need));
+        *have = need;
+        return FP_OK;
+    };
+    int rc;
+    if (M.n_layers == 4 && M.h_dims[1] == TC_H && M.h_dims[2] == TC_H && M.h_dims[3] == TC_H && !C.tc_frags)
+        FP_CUDA_OK(ctx, cudaMalloc((void**)&C.tc_frags, (size_t)TC_FRAGS * sizeof(float4) + (size_t)TC_MISC * sizeof(float)));
+    bool wide = M.n_layers >= 2;
+    for (int l = 1; l < M.n_layers && wide; ++l) wide = M.h_dims[l] == WD_H;
+    if (wide) {
+        const size_t mbytes = (size_t)wd_misc_floats(M.n_layers) * sizeof(float);
+        if ((rc = ensure(&C.w5_blob, &C.w5_bytes, w5_blob_bytes(M.n_layers) + mbytes)) != FP_OK) return rc;
+        if ((rc = ensure((void**)&C.wd_frags, &C.wd_bytes, wd_frag_total(M.n_layers) * sizeof(uint4) + mbytes)) != FP_OK) return rc;
+    }
+    size_t blob_bytes = C.blob_floats * sizeof(float);
+    if ((rc = ensure((void**)&C.blob, &blob_bytes, (size_t)off * sizeof(float))) != FP_OK) return rc;
+    C.blob_floats = blob_bytes / sizeof(float);
+    return FP_OK;
+}
+
 int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell, const fp_mlp* h_mlp,
                     float relax_w, float* coef, uint32_t* flags, bool with_update_constants, cudaStream_t st)
 {
@@ -244,7 +281,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         P.theta_ref = M.theta_ref; P.relax_w = relax_w;
         P.dt = ctx->p.dt; P.eps2_scale = ctx->p.eps2_scale; P.cellc = cellc;
         const size_t smem = fbytes + (size_t)TC_WARPS * 16 * 17 * sizeof(float);
-        static int occ = 0;
+        int& occ = ctx->mlp_tc_occ;
         if (occ == 0) {
             FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mlp_tc_kernel, TC_THREADS, smem);
@@ -282,7 +319,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         P.dt = ctx->p.dt; P.eps2_scale = ctx->p.eps2_scale; P.cellc = cellc;
         const size_t smem = (size_t)2 * W5_A_PART + (size_t)W5_STAGES * W5_STAGE_BYTES +
                             (size_t)((wd_misc_floats(M.n_layers) + 3) & ~3) * sizeof(float) + 16 * sizeof(uint64_t);
-        static bool attr5_set = false;
+        bool& attr5_set = ctx->mlp_attr_w5;
         if (!attr5_set) {
             FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_wide5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
             attr5_set = true;
@@ -313,7 +350,7 @@ int fpi_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const fl
         P.dt = ctx->p.dt; P.eps2_scale = ctx->p.eps2_scale; P.cellc = cellc;
         const size_t smem = (size_t)4 * WD_M * WD_XS * sizeof(__nv_bfloat16) +
                             (size_t)((wd_misc_floats(M.n_layers) + 3) & ~3) * sizeof(float) + (size_t)WD_M * 17 * sizeof(float);
-        static bool attr_set = false;
+        bool& attr_set = ctx->mlp_attr_wd;
         if (!attr_set) {
             FP_CUDA_OK(ctx, cudaFuncSetAttribute(mlp_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
             attr_set = true;

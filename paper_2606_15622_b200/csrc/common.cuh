@@ -58,10 +58,17 @@ struct fp_ctx {
     uint32_t *bin_total = nullptr;   // [bins]
     size_t    block_hist_elems = 0;
     float    *cellc = nullptr;       // [ncell * 28] per-cell constants of the velocity update (update.cu)
-    double   *mom_acc = nullptr;     // [ncell * 28] raw-sum accumulators of the high-ppc gather (moments_seg.cuh), lazy
-    size_t    mom_acc_bytes = 0;
-    double   *upd_acc = nullptr;     // [ncell * 6] per-cell sums of the high-ppc update (update_seg.cuh), lazy
-    size_t    upd_acc_bytes = 0;
+    double   *mom_acc = nullptr;     // [ncell * 28] raw-sum accumulators of the high-ppc gather (moments_seg.cuh)
+    double   *upd_acc = nullptr;     // [ncell * 6] per-cell sums of the high-ppc update (update_seg.cuh)
+    // sticky device-side state check (cell_start not a monotone prefix ending at np): one word of mapped pinned host
+    // memory that kernels OR into and every entry point reads without synchronising
+    uint32_t *h_err = nullptr, *d_err = nullptr;
+    uint32_t *d_errdev = nullptr;    // device-memory copy of the word for kernels that must not run on bad boundaries
+    int       mom_occ[6] = {0, 0, 0, 0, 0, 0};       // resident CTAs per SM of moments_warp_kernel<2^k, *>
+    int       mlp_tc_occ = 0;
+    bool      mlp_attr_w5 = false, mlp_attr_wd = false;
+    // test / measurement switches read from the environment once, at fp_create
+    bool      env_mom_seg = false, env_mom_no_seg = false, env_upd_seg = false, env_upd_no_seg = false;
     bool      upd_attr[4] = {false, false, false, false};   // shared-memory attribute set for update_warp_kernel<4|8|16|32> (per context, i.e. per device)
     // fp_step_host staging (allocated lazily)
     float    *hs_f[2][5] = {{nullptr}};
@@ -97,6 +104,19 @@ static inline int fp_fail(fp_ctx* ctx, int code, const char* msg)
 {
     if (ctx) { snprintf(ctx->err, sizeof(ctx->err), "%s", msg); }
     return code;
+}
+
+// bits of the device-side state word (fp_ctx::h_err)
+#define FP_DEVERR_CELL_START 1u      // cell_start is not a monotone prefix sum ending at np
+// read the sticky state word at the entry of a call (no synchronisation: the word lives in mapped host memory)
+static inline int fp_state_check(fp_ctx* ctx, const char* who)
+{
+    if (ctx->h_err && *(volatile uint32_t*)ctx->h_err) {
+        snprintf(ctx->err, sizeof(ctx->err), "%s: an earlier call on this context found cell_start not to be a monotone prefix sum "
+                 "ending at np; its cells were skipped (call fp_check to clear)", who);
+        return FP_ERR_STATE;
+    }
+    return FP_OK;
 }
 
 #define FP_CUDA_OK(ctx, call)                                                                        \
@@ -197,6 +217,34 @@ __device__ __forceinline__ float2 fpd_fma2(float2 a, float2 b, float2 c) { retur
 __device__ __forceinline__ float2 fpd_mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 fpd_add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 fpd_dup(float a) { return make_float2(a, a); }
+
+// The cell boundaries a warp is about to use: lane i holds cell_start[min(c0 + i, ncell)], cells c0 .. c0 + ncells - 1 are the
+// warp's.  They must be monotone, lie in [0, np], and cell_start[ncell] must be np.  A violation sets the context's
+// state word (FP_ERR_STATE at the next entry point); the caller then treats the cells as empty.
+__device__ __forceinline__ bool fpd_cells_ok(int32_t cs, int64_t c0, int ncells, int32_t ncell, int64_t np, int lane,
+                                             uint32_t* __restrict__ err)
+{
+    const int32_t nxt = __shfl_down_sync(0xffffffffu, cs, 1);
+    const bool mine = lane <= ncells;
+    const bool bad = mine && (cs < 0 || (int64_t)cs > np || (lane < ncells && nxt < cs) ||
+                              (c0 + lane >= ncell && (int64_t)cs != np));
+    const bool ok = !__any_sync(0xffffffffu, bad);
+    if (!ok && lane == 0 && err) atomicOr(err, FP_DEVERR_CELL_START);
+    return ok;
+}
+
+// Stand-alone version of the same check for the paths that walk cell_start by binary search (moments_seg, update_seg)
+static __global__ void fp_cs_check_kernel(const int32_t* __restrict__ cell_start, int32_t ncell, int64_t np, uint32_t* __restrict__ err,
+                                          uint32_t* __restrict__ err_dev)
+{
+    fpd_pdl();
+    bool bad = false;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i <= ncell; i += (int64_t)gridDim.x * blockDim.x) {
+        const int32_t v = cell_start[i];
+        bad |= v < 0 || (int64_t)v > np || (i < ncell && cell_start[i + 1] < v) || (i == ncell && (int64_t)v != np);
+    }
+    if (bad) { atomicOr(err, FP_DEVERR_CELL_START); atomicOr(err_dev, FP_DEVERR_CELL_START); }
+}
 
 // 64-bit shuffle helpers
 __device__ __forceinline__ double fpd_shfl_xor(double v, int mask)

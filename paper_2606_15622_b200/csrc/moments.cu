@@ -170,6 +170,9 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
 // (v - v_pivot) - m again; (iii) per-lane sums stay fp32 for the whole cell (<= 64 terms per packed half, as in the
 // chunked path) and go straight to the cross-lane tree.  `after_reads` runs once the staging buffer is not needed
 // any more.  Lanes of different groups run different trip counts; the (masked) last step is peeled.
+#ifndef MOM_F32MEAN
+#define MOM_F32MEAN 1
+#endif
 template <int G, bool FULL, class Hook>
 __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,
                                              bool have, int gl, int group, double* __restrict__ rec, Hook after_reads)
@@ -216,6 +219,20 @@ __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, c
         A1 = fpd_fma2(fpd_add2(make_float2(y[q0], y[q1]), npy), msk, A1);
         A2 = fpd_fma2(fpd_add2(make_float2(z[q0], z[q1]), npz), msk, A2);
     }
+#if MOM_F32MEAN
+    // the mean in fp32: <= 64 thermal-sized terms per packed half, a balanced tree over the lanes, n < 2^24 exact and its
+    // reciprocal correctly rounded: ~1e-7 of the thermal speed on U, far below that on the central moments
+    float S0 = A0.x + A0.y, S1 = A1.x + A1.y, S2 = A2.x + A2.y;
+#pragma unroll
+    for (int d = G / 2; d >= 1; d >>= 1) {
+        S0 += __shfl_xor_sync(0xffffffffu, S0, d); S1 += __shfl_xor_sync(0xffffffffu, S1, d);
+        S2 += __shfl_xor_sync(0xffffffffu, S2, d);
+    }
+    const float invnf = n > 0 ? __frcp_rn((float)n) : 0.0f;
+    const float m0f = S0 * invnf, m1f = S1 * invnf, m2f = S2 * invnf;
+    const double invn = (double)invnf, m0d = (double)m0f, m1d = (double)m1f, m2d = (double)m2f;
+    const float2 nm0 = fpd_dup(-m0f), nm1 = fpd_dup(-m1f), nm2 = fpd_dup(-m2f);
+#else
     double S0 = (double)A0.x + (double)A0.y, S1 = (double)A1.x + (double)A1.y, S2 = (double)A2.x + (double)A2.y;
 #pragma unroll
     for (int d = G / 2; d >= 1; d >>= 1) {
@@ -224,6 +241,7 @@ __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, c
     const double invn = n > 0 ? 1.0 / (double)n : 0.0;
     const double m0d = S0 * invn, m1d = S1 * invn, m2d = S2 * invn;
     const float2 nm0 = fpd_dup(-(float)m0d), nm1 = fpd_dup(-(float)m1d), nm2 = fpd_dup(-(float)m2d);
+#endif
     // ---- pass 2: central moments
     float2 P[6], T[10], F[6], Gm[3];
 #pragma unroll
@@ -440,7 +458,7 @@ template <int G, bool FULL>
 __global__ void __launch_bounds__(MOM_THREADS, MOM_MINB)
 moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
                     const int32_t* __restrict__ cell_start, int32_t ncell, int64_t np, int32_t aligned,
-                    double* __restrict__ mom)
+                    double* __restrict__ mom, uint32_t* __restrict__ err)
 {
     fpd_pdl();
     constexpr int NREC = FULL ? 29 : 13;
@@ -459,7 +477,11 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
     uint64_t* wbar = bars + warp * 2;
     if (lane == 0) { fpt_mbar_init(&wbar[0], 1); fpt_mbar_init(&wbar[1], 1); }
     __syncwarp();
-    auto load_cs = [&](int64_t c) { return cell_start[min(c * CPW + lane, (int64_t)ncell)]; };
+    auto load_cs = [&](int64_t c) {                      // the chunk's cell boundaries, validated (empty chunk if invalid)
+        const int32_t v = cell_start[min(c * CPW + lane, (int64_t)ncell)];
+        const int cells = (int)min((int64_t)CPW, (int64_t)ncell - c * CPW);
+        return fpd_cells_ok(v, c * CPW, cells, ncell, np, lane, err) ? v : 0;
+    };
     auto range_of = [&](int32_t cs) {
         return fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, aligned != 0, MOM_CAP);
     };
@@ -486,7 +508,8 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
         if (more) {
             r_nxt = range_of(cs_nxt);
             if (NST == 2) {
-                __syncwarp();                               // every lane is done reading buffer b^1 (previous chunk)
+                fpt_fence_proxy_async();                    // generic-proxy writes to buffer b^1 (tail particles, scratch) vs the bulk copy
+                __syncwarp();                               // every lane is done with buffer b^1 (previous chunk)
                 issue(r_nxt, b ^ 1);
             }
         }
@@ -560,7 +583,7 @@ static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float
     const int cells_per_block = MOM_WARPS * (32 / G);
     const int aligned = ((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0 ? 1 : 0;
     const size_t smem = (size_t)MOM_WARPS * MOM_STAGES * 3 * MOM_CAP * sizeof(float) + MOM_WARPS * 2 * sizeof(uint64_t);
-    static int occ = 0;                           // resident CTAs per SM, one value per instantiation (G)
+    int& occ = ctx->mom_occ[G == 2 ? 0 : G == 4 ? 1 : G == 8 ? 2 : G == 16 ? 3 : 4];   // resident CTAs per SM
     if (occ == 0) {
         cudaFuncSetAttribute(moments_warp_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         cudaFuncSetAttribute(moments_warp_kernel<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -570,8 +593,8 @@ static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float
     const int want = fp_div_up(ctx->ncell, cells_per_block);
     const int cap = ctx->num_sms * occ;
     const int blocks = want < cap ? want : cap;
-    if (mode) fp_launch(moments_warp_kernel<G, true>, blocks, MOM_THREADS, smem, st, vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
-    else      fp_launch(moments_warp_kernel<G, false>, blocks, MOM_THREADS, smem, st, vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom);
+    if (mode) fp_launch(moments_warp_kernel<G, true>, blocks, MOM_THREADS, smem, st, vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom, ctx->d_err);
+    else      fp_launch(moments_warp_kernel<G, false>, blocks, MOM_THREADS, smem, st, vx, vy, vz, cell_start, ctx->ncell, np, aligned, mom, ctx->d_err);
 }
 
 extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
@@ -580,6 +603,7 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     if (!ctx) return FP_ERR_ARG;
     if (np < 0 || !cell_start || !mom || (mode != 0 && mode != 1)) return fp_fail(ctx, FP_ERR_ARG, "fp_cell_moments: bad argument");
     if (np > 0 && (!vx || !vy || !vz)) return fp_fail(ctx, FP_ERR_ARG, "fp_cell_moments: null velocity pointer");
+    if (fp_state_check(ctx, "fp_cell_moments") != FP_OK) return FP_ERR_STATE;
     cudaStream_t st = (cudaStream_t)stream;
     const double ppc = (double)np / (double)ctx->ncell;
     // group width: the chunk of 32/G cells must fit the staging buffer (tiles.cuh)
@@ -587,27 +611,23 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     const bool aligned16 = ((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0;
     // (with at least one resident warp's worth of cells per warp slot, one warp per huge cell is still the faster
     // path: 4096 cells x 1000 particles 39 vs 46 us; 300 cells x 30,000 particles 367 vs 60 us)
-    const bool few_cells = ctx->ncell < ctx->num_sms * 16 || getenv("FPCL_MOM_SEG") != nullptr;
-    if (ppc > MOM_SEG_MIN && few_cells && aligned16 && np > 0 && np < ((int64_t)1 << 31) && !getenv("FPCL_MOM_NO_SEG")) {
-        const size_t bytes = (size_t)ctx->ncell * 28 * sizeof(double);
-        if (ctx->mom_acc_bytes < bytes) {
-            if (ctx->mom_acc) cudaFree(ctx->mom_acc);
-            ctx->mom_acc = nullptr; ctx->mom_acc_bytes = 0;
-            FP_CUDA_OK(ctx, cudaMalloc((void**)&ctx->mom_acc, bytes));
-            ctx->mom_acc_bytes = bytes;
-        }
+    const bool few_cells = ctx->ncell < ctx->num_sms * 16 || ctx->env_mom_seg;
+    if (ppc > MOM_SEG_MIN && few_cells && aligned16 && np > 0 && np < ((int64_t)1 << 31) && !ctx->env_mom_no_seg) {
+        const size_t bytes = (size_t)ctx->ncell * 28 * sizeof(double);       // allocated at fp_create
+        fp_launch(fp_cs_check_kernel, fp_div_up(ctx->ncell + 1, 256) < 296 ? fp_div_up(ctx->ncell + 1, 256) : 296, 256, 0, st, cell_start,
+                  ctx->ncell, np, ctx->d_err, ctx->d_errdev);
         FP_CUDA_OK(ctx, cudaMemsetAsync(ctx->mom_acc, 0, bytes, st));
         const int64_t nslices = (np + MOM_SEG - 1) / MOM_SEG;
         const int64_t want = (nslices + MOM_SEG_WARPS - 1) / MOM_SEG_WARPS;
         const int cap = ctx->num_sms * 8;
         fp_launch(mom_seg_kernel, (int)(want < cap ? want : cap), MOM_SEG_WARPS * 32, 0, st, vx, vy, vz, cell_start,
-                  ctx->ncell, np, ctx->mom_acc);
+                  ctx->ncell, np, ctx->mom_acc, (const uint32_t*)ctx->d_errdev);
         if (mode) fp_launch(mom_seg_finalize_kernel<true>, fp_div_up(ctx->ncell, 128), 128, 0, st, vx, vy, vz, cell_start,
-                            ctx->ncell, (const double*)ctx->mom_acc, mom);
+                            ctx->ncell, (const double*)ctx->mom_acc, mom, (const uint32_t*)ctx->d_errdev);
         else      fp_launch(mom_seg_finalize_kernel<false>, fp_div_up(ctx->ncell, 128), 128, 0, st, vx, vy, vz, cell_start,
-                            ctx->ncell, (const double*)ctx->mom_acc, mom);
+                            ctx->ncell, (const double*)ctx->mom_acc, mom, (const uint32_t*)ctx->d_errdev);
         FP_LAUNCH_OK(ctx);
-        FP_COUNT(ctx, 2);
+        FP_COUNT(ctx, 3);
         return FP_OK;
     }
     // lanes per cell: the smallest G whose chunk of 32/G mean-sized cells leaves room for the count fluctuations

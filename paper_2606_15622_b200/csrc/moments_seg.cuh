@@ -54,9 +54,11 @@ __device__ __forceinline__ void mom_seg_pivot(const float* __restrict__ vx, cons
 
 __global__ void __launch_bounds__(MOM_SEG_WARPS * 32)
 mom_seg_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
-               const int32_t* __restrict__ cell_start, int32_t ncell, int64_t np, double* __restrict__ acc)
+               const int32_t* __restrict__ cell_start, int32_t ncell, int64_t np, double* __restrict__ acc,
+               const uint32_t* __restrict__ err_dev)
 {
     fpd_pdl();
+    if (*err_dev) return;                                   // cell_start failed fp_cs_check_kernel: touch nothing
     __shared__ __align__(16) float stage[MOM_SEG_WARPS][3][MOM_SEG];
     __shared__ __align__(8) uint64_t bars[MOM_SEG_WARPS];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -142,9 +144,10 @@ template <bool FULL>
 __global__ void __launch_bounds__(128)
 mom_seg_finalize_kernel(const float* __restrict__ vx, const float* __restrict__ vy, const float* __restrict__ vz,
                         const int32_t* __restrict__ cell_start, int32_t ncell, const double* __restrict__ acc,
-                        double* __restrict__ mom)
+                        double* __restrict__ mom, const uint32_t* __restrict__ err_dev)
 {
     fpd_pdl();
+    if (*err_dev) return;
     constexpr int NREC = FULL ? 29 : 13;
     const int cell = blockIdx.x * blockDim.x + threadIdx.x;
     if (cell >= ncell) return;

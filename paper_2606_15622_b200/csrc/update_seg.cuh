@@ -28,9 +28,10 @@ __device__ __forceinline__ int32_t upd_seg_first_cell(const int32_t* __restrict_
 __global__ void __launch_bounds__(UPD_SEG_WARPS * 32)
 upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
                  const int32_t* __restrict__ cell_start, int64_t np, const float* __restrict__ cellc,
-                 double* __restrict__ acc, const __grid_constant__ upd_params Q)
+                 double* __restrict__ acc, const uint32_t* __restrict__ err_dev, const __grid_constant__ upd_params Q)
 {
     fpd_pdl();
+    if (*err_dev) return;                                   // cell_start failed fp_cs_check_kernel: touch nothing
     __shared__ __align__(16) float stage[UPD_SEG_WARPS][4][UPD_SEG];
     __shared__ __align__(8) uint64_t bars[UPD_SEG_WARPS];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -103,9 +104,11 @@ upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restri
 __global__ void __launch_bounds__(UPD_SEG_WARPS * 32)
 upd_seg_b_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz,
                  const int32_t* __restrict__ cell_start, int64_t np, const float* __restrict__ cellc,
-                 const double* __restrict__ acc, uint32_t* __restrict__ flags, const __grid_constant__ upd_params Q)
+                 const double* __restrict__ acc, uint32_t* __restrict__ flags, const uint32_t* __restrict__ err_dev,
+                 const __grid_constant__ upd_params Q)
 {
     fpd_pdl();
+    if (*err_dev) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t nslices = (np + UPD_SEG - 1) / UPD_SEG;
     for (int64_t sl = (int64_t)blockIdx.x * UPD_SEG_WARPS + warp; sl < nslices; sl += (int64_t)gridDim.x * UPD_SEG_WARPS) {

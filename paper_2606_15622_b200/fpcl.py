@@ -20,7 +20,7 @@ FLAG_EMPTY, FLAG_LOWCOUNT, FLAG_SINGULAR, FLAG_ILLCOND, FLAG_ALPHA, FLAG_SKIPPED
 EXPORTS = ["fp_create", "fp_destroy", "fp_last_error", "fp_version", "fp_sort_by_cell", "fp_cell_moments",
            "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host",
            "fp_timing_enable", "fp_timing_read", "fp_launch_count", "fp_set_mlp_tensor_cores", "fp_cell_diagnostics",
-           "fp_average_results", "fp_cell_sixth_moment"]
+           "fp_average_results", "fp_cell_sixth_moment", "fp_reserve", "fp_check"]
 NSTAGES = 6
 STAGE_NAMES = ["stream_walls", "sort_keys", "gather", "moments", "closure", "update"]
 
@@ -82,6 +82,8 @@ def load(path=None):
     lib.fp_timing_read.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32)]
     lib.fp_launch_count.argtypes = [vp]
     lib.fp_set_mlp_tensor_cores.argtypes = [vp, i32]
+    lib.fp_reserve.argtypes = [vp, C.POINTER(FpMlp), i32]
+    lib.fp_check.argtypes = [vp, vp]
     for name in EXPORTS:
         if name not in ("fp_last_error", "fp_version", "fp_launch_count"):
             getattr(lib, name).restype = C.c_int
@@ -257,6 +259,15 @@ def fp_set_mlp_tensor_cores(ctx, enable):
 
 def fp_launch_count(ctx):
     return int(load().fp_launch_count(ctx))
+
+
+def fp_reserve(ctx, mlp=None, host_staging=False):
+    _check(ctx, load().fp_reserve(ctx, C.byref(mlp.c_struct) if mlp is not None else None, int(bool(host_staging))),
+           "fp_reserve")
+
+
+def fp_check(ctx):
+    _check(ctx, load().fp_check(ctx, _stream()), "fp_check")
 
 
 # ---------------------------------------------------------------------------------------------- conveniences

@@ -268,6 +268,75 @@ def test_step_host(gpu, wl, orc):
     ctx.close()
 
 
+def test_step_host_pinned_large_with_walls(gpu, wl):
+    """fp_step_host with PINNED host buffers and 1M particles at a large time step (many wall re-emissions, which
+    rewrite vx, vy, vz in the stream kernel): bit-identical to the device-resident fp_step.  Guards the ordering of the
+    uploads against the first kernel (a vz copy still in flight used to be able to overwrite the re-drawn vz)."""
+    import torch
+    cfg, st = wl.cavity(n=100, ppc=100, seed=12)
+    cfg["dt"] = float(np.float32(0.02))                                  # ~2 cells per step: a few percent hit a wall
+    ctx = gpu.Context(cfg)
+    gpu.fp_reserve(ctx.h, None, True)                                    # staging buffers up front
+    a = gpu.to_device(st)
+    b = {k: torch.empty_like(v) for k, v in a.items()}
+    out = ctx.alloc_step_outputs(0)
+    ctx.step(a, b, 3, out, closure=0)
+    want = gpu.to_host(b)
+    moved = (np.abs(st["vz"][want["pid"]] - want["vz"]) > 0).mean()
+    h = {k: torch.from_numpy(np.ascontiguousarray(v).copy()).pin_memory() for k, v in st.items() if k != "pid"}
+    h["pid"] = torch.from_numpy(st["pid"].view(np.int32).copy()).pin_memory()
+    for rep in range(3):                                                 # a race would not show every time
+        for k, v in st.items():
+            h[k].copy_(torch.from_numpy(v.view(np.int32) if k == "pid" else v))
+        hn = {k: (v.numpy().view(np.uint32) if k == "pid" else v.numpy()) for k, v in h.items()}
+        ctx.step_host(hn, 3, closure=0)
+        for k in ("x", "y", "vx", "vy", "vz", "pid"):
+            assert np.array_equal(_bits(hn[k]), _bits(want[k])), (k, rep)
+    assert moved > 0.9                                                   # the update touched the velocities at all
+    ctx.close()
+
+
+def test_unsorted_cell_start_is_a_state_error(gpu, wl):
+    """cell_start that is not a monotone prefix ending at np: the cells concerned are skipped on the device, the sticky
+    state word makes the NEXT entry point return FP_ERR_STATE, fp_check reports and clears it (include/fpcl.h)."""
+    import torch
+    cfg, st = wl.cavity(n=12, ppc=40, seed=4)
+    ctx = gpu.Context(cfg)
+    a = gpu.to_device(st)
+    b = {k: torch.empty_like(v) for k, v in a.items()}
+    out = ctx.alloc_step_outputs(0)
+    ctx.step(a, b, 0, out, closure=0)
+    cs = out["cell_start"].clone()
+    good = ctx.cell_moments(b["vx"], b["vy"], b["vz"], cs, 1)
+    gpu.fp_check(ctx.h)                                                  # clean so far
+    for kind in ("swap", "end", "negative"):
+        bad = cs.clone()
+        if kind == "swap":
+            bad[40], bad[41] = cs[41] + 7, cs[40]
+        elif kind == "end":
+            bad[-1] = cs[-1] - 1
+        else:
+            bad[5] = -3
+        mom = ctx.cell_moments(b["vx"], b["vy"], b["vz"], bad, 1)        # asynchronous: returns FP_OK
+        torch.cuda.synchronize()
+        assert torch.isfinite(mom).all()
+        with pytest.raises(gpu.FpclError, match="code -2"):
+            ctx.cell_moments(b["vx"], b["vy"], b["vz"], cs, 1)
+        with pytest.raises(gpu.FpclError, match="code -2"):
+            gpu.fp_check(ctx.h)
+        gpu.fp_check(ctx.h)                                              # cleared
+        v = [b[k].clone() for k in ("vx", "vy", "vz")]
+        fl = out["flags"].clone()
+        ctx.velocity_update(v[0], v[1], v[2], b["pid"], bad, good, out["coef"], 9, fl)
+        torch.cuda.synchronize()
+        assert all(torch.isfinite(x).all() for x in v)
+        with pytest.raises(gpu.FpclError, match="code -2"):
+            gpu.fp_check(ctx.h)
+    again = ctx.cell_moments(b["vx"], b["vy"], b["vz"], cs, 1)
+    assert torch.equal(again, good)
+    ctx.close()
+
+
 def test_multi_step_statistics(gpu, wl, orc):
     """100 Couette steps (BASELINE config 1) with each closure: particle count and ids conserved, no non-finite value,
     temperature stays put, and the mean profile agrees with the oracle's own 100-step run statistically."""
