@@ -377,8 +377,10 @@ def couette_small(fpcl, torch, workloads):
 
 def closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak):
     """BASELINE config 2: 100x100 cells x 50 particles from a Grad-13-perturbed Maxwellian (seed 1), no streaming:
-    moment gather, exact closure and surrogate timed separately (cold L2), flag counts and the condition estimates
-    of the exact closure (50 ppc makes some cells ill-conditioned by design)."""
+    moment gather, exact closure and surrogate timed separately (cold L2), flag counts and a histogram of the exact
+    closure's condition estimates.  With |s_ij| <= 0.3, |q| <= 0.2 and 50 particles per cell this recipe stays well
+    conditioned (kappa_1 <= ~1e2 with the eps^2 term of reading R2-e); the ill-conditioned half of the closure contract
+    (kappa up to 1e16, singular cells) is exercised by tests/test_gpu_parity.py::test_closure_exact_conditioning."""
     cfg, st = workloads.grad13_cells()[:2]
     ctx = fpcl.Context(cfg)
     srt, cs, _ = ctx.sort_by_cell(fpcl.to_device(st), want_perm=False)
@@ -388,7 +390,7 @@ def closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak):
     coef, flags, kappa = ctx.closure_exact(mom, want_kappa=True)
     kap = kappa.cpu().numpy()
     fl = flags.cpu().numpy().view(np.uint32)
-    edges = [0.0, 1e2, 1e3, 1e4, 1e6, 1e8, float("inf")]
+    edges = [0.0, 10.0, 20.0, 40.0, 80.0, 160.0, 1e3, 1e4, 1e6, 1e8, float("inf")]
     hist, _ = np.histogram(kap[kap > 0], bins=edges)
     res = {"particles": int(srt["x"].numel()), "cells": ctx.ncell, "kernels_cold_l2": tab,
            "flag_counts": {"illcond": int((fl & 8 != 0).sum()), "singular": int((fl & 4 != 0).sum()),

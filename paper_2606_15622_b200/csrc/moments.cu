@@ -171,7 +171,7 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
 // chunked path) and go straight to the cross-lane tree.  `after_reads` runs once the staging buffer is not needed
 // any more.  Lanes of different groups run different trip counts; the (masked) last step is peeled.
 #ifndef MOM_F32MEAN
-#define MOM_F32MEAN 1
+#define MOM_F32MEAN 0                   // 1: mean by an fp32 tree (2 % fewer instructions, but U then uses 0.8 of its 1e-6 tolerance)
 #endif
 template <int G, bool FULL, class Hook>
 __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,

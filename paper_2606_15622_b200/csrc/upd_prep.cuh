@@ -8,7 +8,8 @@
 //
 // layout of the constants: [0..2] U_hi, [3..5] U_lo, [6..11] B = C + I/tau (11,12,13,22,23,33), [12..14] gamma,
 // [15..17] eps2*h, [18] eps2, [19] 3 theta, [20] E1, [21] (1-E1) tau, [22] sqrt(theta (1-E2)), [23] active,
-// [24] tau^2 (1-E1)^2 / (3 theta), [25] 2 tau (E1-E2) / (3 theta)
+// [24] tau^2 (1-E1)^2 / (3 theta), [25] 2 tau (E1-E2) / (3 theta),
+// [26] |c|^2 beyond which a particle's drift is re-evaluated in fp64 (see upd_far_kernel in update.cu)
 #pragma once
 #include "common.cuh"
 
@@ -45,6 +46,14 @@ __device__ __forceinline__ uint32_t upd_prep_cell(const double* rec, int stride,
     o4[3] = make_float4(cf[6], cf[7], cf[8], (float)(eps2 * h0));
     o4[4] = make_float4((float)(eps2 * h1), (float)(eps2 * h2), (float)eps2, (float)(3.0 * theta));
     o4[5] = make_float4((float)E1, (float)((1.0 - E1) * tau), (float)sqrt(theta * (1.0 - E2)), 1.0f);
-    o4[6] = make_float4((float)(tau * tau * (1.0 - E1) * (1.0 - E1) * i3t), (float)(2.0 * tau * (E1 - E2) * i3t), 0.0f, 0.0f);
+    // [26]: in fp32 a drift term T costs ~6e-8 |T| of absolute error; the quadratic and cubic terms of a particle far out in
+    // the cell's distribution, (1-E1) tau |gamma| c^2 and (1-E1) tau eps2 |c|^3, stay below 3 sqrt(theta) (error < 2e-7
+    // sqrt(theta)) as long as |c|^2 < min(3 s / (kap |gamma|), (3 s / (kap eps2))^(2/3)); never below (5 sigma)^2 = 25 theta,
+    // up to where the terms are a few thermal speeds in any physical state.  Equilibrium cells (eps2, gamma ~ 0): infinity.
+    const double kap = (1.0 - E1) * tau, s3 = 3.0 * sqrt(theta);
+    const double gmax = fmax(fabs((double)cf[6]), fmax(fabs((double)cf[7]), fabs((double)cf[8])));
+    double far2 = fmin(gmax > 0.0 ? s3 / (kap * gmax) : INFINITY, eps2 > 0.0 ? cbrt((s3 / (kap * eps2)) * (s3 / (kap * eps2))) : INFINITY);
+    far2 = fmin(fmax(far2, 25.0 * theta), 3.0e38);
+    o4[6] = make_float4((float)(tau * tau * (1.0 - E1) * (1.0 - E1) * i3t), (float)(2.0 * tau * (E1 - E2) * i3t), (float)far2, 0.0f);
     return 0u;
 }

@@ -232,6 +232,82 @@ def test_closure_exact(gpu, wl, orc, name):
         ctx.close()
 
 
+def _conditioning_ensemble(orc, seed=0):
+    """FULL records whose scaled 9x9 systems have kappa_1 from 1e1 to beyond 1e12, from fp32 particles:
+    (a) 40-particle clouds squeezed towards a plane / a line by a factor 10^-7.5 .. 1 (near-collinear clouds),
+    (b) the same with the squeeze exactly zero and with one component exactly constant (rank-deficient: SINGULAR),
+    (c) low-count cells of 9 .. 14 particles (min_count = 9 lets them through; PAPER.md:564 'low-count outliers'),
+    (d) Grad-13-like clouds as a well-conditioned control."""
+    rng = np.random.default_rng(seed)
+    nc = 4000
+    counts = np.full(nc, 40)
+    counts[3000:3600] = rng.integers(9, 15, 600)
+    sq = 10 ** rng.uniform(-7.5, 0, nc)
+    sq[:50] = 0.0
+    sq[3000:] = 1.0
+    n = int(counts.sum())
+    cs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    seg = np.repeat(np.arange(nc), counts)
+    v = rng.normal(0, 0.7, (n, 3))
+    v[:, 2] *= sq[seg]
+    v[:, 1] *= np.sqrt(sq[seg])
+    v += 0.2 * (rng.exponential(size=(n, 3)) - 1.0) * np.array([1.0, 1.0, 1.0]) * np.minimum(sq[seg], 1.0)[:, None]
+    v += rng.uniform(-0.3, 0.3, (nc, 3))[seg]
+    v[seg < 25, 2] = 0.25
+    v = v.astype(np.float32)
+    return orc.cell_moments(v[:, 0], v[:, 1], v[:, 2], cs, 1), nc, n
+
+
+def test_closure_exact_conditioning(gpu, wl, orc):
+    """The ill-conditioned half of the a4 contract (north_star: 1e-5 'on cells with condition number < 1e8 (flagged
+    otherwise)'; PAPER.md:564 says such cells occur).  Same fp64 records to both sides."""
+    import torch
+    mom, nc, n = _conditioning_ensemble(orc)
+    min_count = 9
+    tau = np.random.default_rng(5).uniform(0.3, 3.0, size=nc).astype(np.float32)
+    ref, rfl, kappa = orc.closure_exact(mom, tau, 1.0, min_count)
+    cfg = wl.make_config(nc, 1, 1.0 / nc, 1.0, 0.01, 1.0, wl.NO_WALLS, max_particles=n, min_count=min_count)
+    ctx = gpu.Context(cfg)
+    coef, fl, kest = ctx.closure_exact(torch.from_numpy(mom).cuda(), torch.from_numpy(tau).cuda(), want_kappa=True)
+    coef, fl, kest = coef.cpu().numpy(), fl.cpu().numpy().view(np.uint32), kest.cpu().numpy()
+    hard = orc.FLAG_EMPTY | orc.FLAG_LOWCOUNT | orc.FLAG_SINGULAR
+    sing = (rfl & orc.FLAG_SINGULAR) != 0
+    solved = (rfl & hard) == 0
+    # the ensemble does what it is for
+    decades = np.histogram(np.log10(kappa[solved]), bins=[0, 2, 4, 6, 8, 10, 12, 17])[0]
+    assert (decades >= 100).all(), decades
+    assert sing.sum() >= 50 and int((rfl & orc.FLAG_ILLCOND != 0).sum()) >= 500
+    # hard flags identical, SINGULAR cells are exactly the Langevin coefficients
+    assert np.array_equal(fl & hard, rfl & hard)
+    lang = np.zeros((nc, 9), np.float32)
+    lang[:, [0, 3, 5]] = (-1.0 / tau.astype(np.float64)).astype(np.float32)[:, None]
+    assert np.array_equal(coef[sing].view(np.uint32), lang[sing].view(np.uint32))
+    # coefficients: max(1e-5, 10 kappa eps) relative, per cell, below the oracle's kappa < 1e8 line ...
+    theta = _theta(mom)
+    well = solved & (kappa < 1e8)
+    worst = 0.0
+    for lo in (0, 2, 4, 6):
+        m = well & (kappa >= 10.0 ** lo) & (kappa < 10.0 ** (lo + 2))
+        tol = max(1e-5, 10.0 * 10.0 ** (lo + 2) * 2.2e-16)
+        worst = max(worst, coef_ratio(coef, ref, tau, theta, tol, mask=m))
+    # ... and, as a report only, above it (both sides solve in fp64; the fp32 store dominates)
+    r_ill = coef_ratio(coef, ref, tau, theta, 1e-5, mask=solved & ~well)
+    # the estimate that decides FP_FLAG_ILLCOND: within a factor 4 of the oracle's exact kappa_1, and a superset of its flags
+    ratio = kest[solved] / kappa[solved]
+    gpu_ill = (fl & orc.FLAG_ILLCOND) != 0
+    orc_ill = (rfl & orc.FLAG_ILLCOND) != 0
+    print("closure conditioning: cells per 2 decades of kappa %s, %d singular; worst err/allowed %.3g below 1e8, %.3g above; "
+          "estimate/kappa in [%.2f, %.2f]; ILLCOND oracle %d, GPU %d (superset: %s)"
+          % (decades.tolist(), int(sing.sum()), worst, r_ill, ratio.min(), ratio.max(), int(orc_ill.sum()), int(gpu_ill.sum()),
+             bool((gpu_ill | ~orc_ill).all())))
+    assert worst <= 1.0
+    assert ratio.min() >= 0.25 and ratio.max() <= 4.0
+    assert (gpu_ill | ~orc_ill).all()
+    assert not gpu_ill[solved & (kappa < 5e6)].any()
+    assert np.isfinite(coef).all()
+    ctx.close()
+
+
 def test_closure_exact_langevin(gpu, wl):
     """Exact Maxwellian moments give c = -delta/tau, gamma = 0 (Eq. 4 :77)."""
     import torch

@@ -211,8 +211,10 @@ def test_step_one(gpu, wl, orc, name, closure):
     touched[orc.cell_index(mid["x"][hit], mid["y"][hit], cfg)] = True
     pre, pre_cs, _ = orc.sort_by_cell(mid, cfg)               # the oracle's sorted pre-update particles
     am = abs_moments(pre["vx"], pre["vy"], pre["vz"], pre_cs, aux["mom"])
-    rm = max(moment_ratio(res["mom"], aux["mom"], 1e-6, absmom=am, mask=~touched),
-             moment_ratio(res["mom"], aux["mom"], 1e-5, absmom=am, mask=touched))
+    rm0 = moment_ratio(res["mom"], aux["mom"], 1e-6, absmom=am, mask=~touched)
+    rm1 = moment_ratio(res["mom"], aux["mom"], 1e-5, absmom=am, mask=touched)
+    rm = max(rm0, rm1)
+    delta_mom = np.where(touched, rm1 * 1e-5, rm0 * 1e-6)      # measured relative mismatch of the two sides' moments
     assert rm <= 1.0
     theta = _theta(aux["mom"])
     tau = cfg["tau"] if tau_fn is None else tau_fn(aux["mom"][:, 0])
@@ -220,11 +222,14 @@ def test_step_one(gpu, wl, orc, name, closure):
     gflags = res["flags"].view(np.uint32)
     assert np.array_equal(gflags & hard, aux["flags"] & hard)
     if closure == 0:
-        # the two closures start from moments that differ by ~1e-7: the coefficient tolerance widens with kappa
-        # (SURVEY 8(c) S3-d); the velocity tolerance follows because the drift term is (1 - E1) tau N ~ 0.1 |c|
+        # the two closures start from moments that differ by delta_mom (measured above, ~1e-7): per cell the coefficient
+        # tolerance is max(1e-5, 30 kappa delta_mom) on every cell below the kappa < 1e8 line.  (SURVEY 8(c) S3-d wrote
+        # 10 kappa delta_mom; the perturbation bound is |dy|/|y| <= kappa (|dA|/|A| + |db|/|b|) = 2 kappa delta in one
+        # norm, and delta_mom is measured per entry against its own scale while kappa_1 is a 1-norm quantity of a 9x9
+        # system: up to another factor 9.  Measured: 11 kappa delta_mom on the cavity, hence 30.)
         _, _, kappa = orc.closure_exact(aux["mom"], tau, cfg["eps2_scale"], cfg["min_count"])
-        good = ((aux["flags"] & (hard | orc.FLAG_ILLCOND)) == 0) & (kappa < 1e4)
-        rc = coef_ratio(res["coef"], aux["coef"], tau, theta, 1e-5 * 100, mask=good)
+        good = ((aux["flags"] & (hard | orc.FLAG_ILLCOND)) == 0) & (kappa < 1e8)
+        rc = coef_ratio(res["coef"], aux["coef"], tau, theta, np.maximum(1e-5, 30.0 * kappa * delta_mom), mask=good)
         # Mach-10 shock-band cells have an O(1) cubic term eps2 c^3 tau: the ~1e-7 mismatch of the two sides' moments
         # (U, theta, h, eps2) is amplified ~100x on its way to the velocities (the stage test feeds identical moments)
         tolv = 1e-4 if name == "cylinder" else 2e-5
@@ -372,24 +377,43 @@ def test_multi_step_statistics(gpu, wl, orc):
         ctx.close()
 
 
-# ------------------------------------------------------------------------------------------------ full size (C3)
-def test_full_size_cavity(gpu, wl, orc):
-    """BASELINE config 3 (200x200 cells x 100 ppc = 4M particles): every stage against the oracle on the full
-    arrays, in the launch configuration bench.py times."""
+# ------------------------------------------------------------------------------------------------ full size
+@pytest.mark.parametrize("case", ["c3_4m", "c4_8m", "c5_20m"])
+def test_full_size(gpu, wl, orc, case):
+    """BASELINE configs at their full sizes, every stage against the oracle on the full arrays, in the launch
+    configuration bench.py times: C3 (200x200 cells x 100 ppc = 4M particles), C4 at 200 ppc (8M particles: the packed
+    sort with 23 index bits, G = 16 lanes per cell) and C5 (400x300 cells, 5..400 ppc, ~20M particles: the two-array
+    sort, dense-chunk fall-backs, embedded body, per-cell tau = tau_ref_n / N; PAPER.md:668 audits 8.0e6 particles on
+    this grid)."""
     import torch
-    cfg, st = wl.cavity()
+    tau_fn, kw = None, {}
+    if case == "c3_4m":
+        cfg, st = wl.cavity()
+    elif case == "c4_8m":
+        cfg, st = wl.cavity(n=200, ppc=200, kn=1.0, seed=42)
+    else:
+        cfg, st, _ = wl.cylinder()
+        tau_ref_n = float(np.float32(cfg["tau"] * cfg["ppc_inf"]))
+        tau_default = np.float32(cfg["tau"])
+
+        def tau_fn(N):
+            with np.errstate(divide="ignore", invalid="ignore"):
+                return np.where(N > 0, np.float32(tau_ref_n) / np.maximum(N, 1).astype(np.float32), tau_default).astype(np.float32)
     ctx = gpu.Context(cfg)
+    if tau_fn is not None:
+        kw = dict(tau_mode=1, tau_ref_n=tau_ref_n, tau_cell=torch.empty(ctx.ncell, dtype=torch.float32, device="cuda"))
     a = gpu.to_device(st)
     b = {k: torch.empty_like(v) for k, v in a.items()}
     out = ctx.alloc_step_outputs(0)
-    for it in range(3):                                  # a few steps so that counts are no longer exactly 100
-        ctx.step(a, b, it, out, closure=0)
+    for it in range(3):                                  # a few steps so that counts are no longer the initial ones
+        ctx.step(a, b, it, out, closure=0, **kw)
         a, b = b, a
     h = gpu.to_host(a)
     step_no = 3
-    ctx.step(a, b, step_no, out, closure=0)
+    ctx.step(a, b, step_no, out, closure=0, **kw)
     got = gpu.to_host(b)
     res = {k: v.cpu().numpy() for k, v in out.items()}
+    del a, b
     # oracle, stage by stage, each fed the GPU's own previous-stage output where floating point is involved
     s1 = orc.stream_walls(h, cfg, step_no)
     s2, cs, perm = orc.sort_by_cell(s1, cfg)
@@ -397,26 +421,31 @@ def test_full_size_cavity(gpu, wl, orc):
     assert np.array_equal(got["pid"], s2["pid"])
     assert np.array_equal(_bits(got["x"]), _bits(s2["x"])) and np.array_equal(_bits(got["y"]), _bits(s2["y"]))
     hit = _bits(s1["vx"]) != _bits(h["vx"])
-    print("C3: %d wall re-emissions" % int(hit.sum()))
-    # moments of the GPU's own sorted pre-update velocities (re-emitted ones differ from the oracle's by <= 1e-6)
+    n = np.diff(cs)
+    print("%s: %d particles, %d..%d per cell, %d wall / body re-emissions" % (case, h["x"].shape[0], n.min(), n.max(), int(hit.sum())))
+    # moments of the oracle's sorted pre-update velocities (re-emitted ones differ from the GPU's by <= 1e-6)
     d2 = gpu.to_device(s2)
-    mom_g = ctx.cell_moments(d2["vx"], d2["vy"], d2["vz"], torch.from_numpy(cs).cuda(), 1).cpu().numpy()
+    cs_d = torch.from_numpy(cs).cuda()
+    mom_g = ctx.cell_moments(d2["vx"], d2["vy"], d2["vz"], cs_d, 1).cpu().numpy()
     mom_o = orc.cell_moments(s2["vx"], s2["vy"], s2["vz"], cs, 1)
     rm = moment_ratio(mom_g, mom_o, absmom=abs_moments(s2["vx"], s2["vy"], s2["vz"], cs, mom_o))
-    coef_o, fl_o, kappa = orc.closure_exact(mom_o, cfg["tau"], cfg["eps2_scale"], cfg["min_count"])
-    coef_g, fl_g = ctx.closure_exact(torch.from_numpy(mom_o).cuda())
+    tau = cfg["tau"] if tau_fn is None else tau_fn(mom_o[:, 0])
+    tau_d = None if tau_fn is None else torch.from_numpy(tau).cuda()
+    coef_o, fl_o, kappa = orc.closure_exact(mom_o, tau, cfg["eps2_scale"], cfg["min_count"])
+    coef_g, fl_g = ctx.closure_exact(torch.from_numpy(mom_o).cuda(), tau_d)
+    hard = orc.FLAG_EMPTY | orc.FLAG_LOWCOUNT | orc.FLAG_SINGULAR
+    assert np.array_equal(fl_g.cpu().numpy().view(np.uint32) & hard, fl_o & hard)
     ok = (fl_o & orc.FLAG_ILLCOND) == 0
-    rc = coef_ratio(coef_g.cpu().numpy(), coef_o, cfg["tau"], _theta(mom_o), 1e-5, mask=ok)
+    rc = coef_ratio(coef_g.cpu().numpy(), coef_o, tau, _theta(mom_o), 1e-5, mask=ok)
     c32 = coef_o.astype(np.float32)
-    rvx, rvy, rvz, rfl = orc.velocity_update(s2["vx"], s2["vy"], s2["vz"], s2["pid"], cs, mom_o, c32, cfg["tau"], cfg,
-                                             step_no, fl_o)
+    rvx, rvy, rvz, rfl = orc.velocity_update(s2["vx"], s2["vy"], s2["vz"], s2["pid"], cs, mom_o, c32, tau, cfg, step_no, fl_o)
     flg = torch.from_numpy(fl_o.view(np.int32).copy()).cuda()
-    ctx.velocity_update(d2["vx"], d2["vy"], d2["vz"], d2["pid"], torch.from_numpy(cs).cuda(),
-                        torch.from_numpy(mom_o).cuda(), torch.from_numpy(c32).cuda(), step_no, flg)
+    ctx.velocity_update(d2["vx"], d2["vy"], d2["vz"], d2["pid"], cs_d, torch.from_numpy(mom_o).cuda(),
+                        torch.from_numpy(c32).cuda(), step_no, flg, tau_cell=tau_d)
     rv = velocity_ratio((d2["vx"].cpu().numpy(), d2["vy"].cpu().numpy(), d2["vz"].cpu().numpy()), (rvx, rvy, rvz), cs,
                         _theta(mom_o))
-    print("C3 full size: moments %.3f, closure %.3g (kappa max %.3g, %d ill-conditioned), update %.3f"
-          % (rm, rc, kappa.max(), int((~ok).sum()), rv))
+    print("%s full size: moments %.3f, closure %.3g (kappa max %.3g, %d ill-conditioned), update %.3f"
+          % (case, rm, rc, kappa.max(), int((~ok).sum()), rv))
     assert rm <= 1.0 and rc <= 1.0 and rv <= 1.0
     assert np.array_equal(flg.cpu().numpy().view(np.uint32), rfl)
     for k in ("vx", "vy", "vz"):
