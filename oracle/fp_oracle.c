@@ -34,6 +34,19 @@
 
 #define ORC_PI 3.14159265358979323846
 
+/* The per-cell (moments, closures, update) and per-particle (streaming) loops carry `#pragma omp parallel for`: iterations
+ * are independent and write disjoint outputs, so the result does not depend on the thread count.  The pragmas are
+ * inert unless the file is compiled with -fopenmp (oracle.py does); orc_set_threads picks the count (bench.py times
+ * one thread and all cores). */
+#ifdef _OPENMP
+#include <omp.h>
+void orc_set_threads(int n) { omp_set_num_threads(n > 0 ? n : omp_get_num_procs()); }
+int orc_max_threads(void) { return omp_get_max_threads(); }
+#else
+void orc_set_threads(int n) { (void)n; }
+int orc_max_threads(void) { return 1; }
+#endif
+
 /* per-cell flag bits (interface constants, stated in include/fpcl.h as FP_FLAG_*) */
 #define ORC_FLAG_EMPTY     1u   /* N == 0                                            */
 #define ORC_FLAG_LOWCOUNT  2u   /* N < min_count: Langevin fallback (R3-c)           */
@@ -94,6 +107,7 @@ void orc_cell_moments(const float *vx, const float *vy, const float *vz, const i
                       int32_t ncell, int32_t mode, double *mom)
 {
     const int stride = mode ? 29 : 13;
+#pragma omp parallel for schedule(dynamic, 64)
     for (int32_t cell = 0; cell < ncell; ++cell) {
         double *m = mom + (size_t)cell * stride;
         for (int k = 0; k < stride; ++k) m[k] = 0.0;
@@ -293,6 +307,7 @@ void orc_closure_exact_cell(const double *m, double tau, double eps2_scale, int3
 void orc_closure_exact(int32_t ncell, const double *mom_full, const float *tau_cell, double tau_scalar,
                        double eps2_scale, int32_t min_count, double *coef, uint32_t *flags, double *kappa)
 {
+#pragma omp parallel for schedule(dynamic, 64)
     for (int32_t c = 0; c < ncell; ++c) {
         double tau = tau_cell ? (double)tau_cell[c] : tau_scalar;
         orc_closure_exact_cell(mom_full + (size_t)c * 29, tau, eps2_scale, min_count, coef + (size_t)c * 9,
@@ -448,6 +463,7 @@ void orc_closure_mlp(int32_t ncell, const double *mom, int32_t stride, const flo
                      int32_t act, int32_t feature_set, double n_scale, double theta_ref, int32_t min_count,
                      double relax_w, const double *coef_old, double *coef, uint32_t *flags)
 {
+#pragma omp parallel for schedule(dynamic, 64)
     for (int32_t c = 0; c < ncell; ++c) {
         const double *m = mom + (size_t)c * stride;
         double *out = coef + (size_t)c * 9;
@@ -535,6 +551,7 @@ void orc_velocity_update(int32_t ncell, const int32_t *cell_start, float *vx, fl
                          const float *tau_cell, double tau_scalar, double dt, double eps2_scale,
                          int32_t conserve_mode, uint64_t seed, uint64_t step, uint32_t *flags)
 {
+#pragma omp parallel for schedule(dynamic, 64)
     for (int32_t cell = 0; cell < ncell; ++cell) {
         int64_t s = cell_start[cell], e = cell_start[cell + 1], n = e - s;
         const double *m = mom + (size_t)cell * stride;
@@ -630,6 +647,7 @@ void orc_stream_walls(int64_t np, float *x, float *y, float *vx, float *vy, floa
 {
     float xmin = x0, xmax = x0 + (float)nx * dx, ymin = y0, ymax = y0 + (float)ny * dy;
     float Lx = xmax - xmin, Ly = ymax - ymin;
+#pragma omp parallel for schedule(static)
     for (int64_t p = 0; p < np; ++p) {
         float xp = fmaf(vx[p], dt, x[p]), yp = fmaf(vy[p], dt, y[p]);
         double v[3] = {vx[p], vy[p], vz[p]};

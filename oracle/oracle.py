@@ -23,8 +23,8 @@ def build(force=False):
     """Compile fp_oracle.c with gcc (-O2 -ffp-contract=off so fp32 position arithmetic is not fused)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".%d.tmp" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-shared", "-fPIC",
-                               "-o", tmp, _SRC, "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-fopenmp", "-shared",
+                               "-fPIC", "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -54,6 +54,12 @@ def _i32(a):
 
 def _u32(a):
     return np.ascontiguousarray(a, dtype=np.uint32)
+
+
+def set_threads(n=0):
+    """Threads of the per-cell / per-particle loops (0 = all cores).  Results do not depend on it."""
+    lib().orc_set_threads(C.c_int(int(n)))
+    return int(lib().orc_max_threads())
 
 
 def ncell_of(cfg):
