@@ -627,6 +627,18 @@ void orc_velocity_update(int32_t ncell, const int32_t *cell_start, float *vx, fl
  *   Body (cylinder, centre (cx,cy), radius R): r2 = fmaf(dy,dy,dx*dx) < R*R -> moved radially to
  *   R*1.000001f: s = (R*1.000001f)/sqrtf(r2), x = fmaf(dx, s, cx) (fp32); velocity redrawn about the
  *   outward normal n = (dx,dy)/r, tangent (-n_y, n_x), and z.
+ *   kind 3 (freestream reservoir, reading R11; SURVEY S7 "outer faces are a constant-Np reservoir: a particle leaving is
+ *   re-inserted on the inflow face with a flux-weighted freestream velocity", PAPER.md:545 Mach-10 argon freestream):
+ *   the freestream (theta_inf; U_inf with U_inf,x > 0) is wall[0]'s (theta_w; ux, uy, uz) and the inflow face is xmin.
+ *   A particle that leaves through a kind-3 face is re-inserted at xmin:
+ *     v_x from the flux-weighted drifting half-Maxwellian f(v) ~ v exp(-(v - U)^2 / (2 theta)), v > 0, by acceptance-
+ *       rejection: mu = (U + sqrt(U^2 + 4 theta)) / 2 (the mode of f), candidate v = mu + sqrt(theta) z with
+ *       z = sqrt(-2 ln u0) cos(2 pi u1), accepted iff v > 0 and (v / mu) exp(1 - v / mu) >= u2 (f / proposal, scaled to 1 at
+ *       the mode); attempt a = 0..7 uses the Philox call with stream 16 + a; if all eight are rejected, v = mu;
+ *     v_y = U_y + t1, v_z = U_z + t2 with (t1, t2) = sqrt(theta) sqrt(-2 ln u0) (cos, sin)(2 pi u1) from the call with stream 32;
+ *     position, in fp32 (it decides the cell): x = xmin + u3 * fl(U_x * dt) (the particle entered at a uniformly distributed
+ *       moment of the step), y = fmaf(u2, Ly, ymin) (uniform along the face; 1D: y unchanged), clamped into the domain;
+ *     no further wall of this step applies to it (the body test still does).
  * wall[k] = {kind, theta_w, ux, uy, uz} for k = xmin, xmax, ymin, ymax, given as 5 doubles each (kind as a number).
  * ------------------------------------------------------------------------------------------------ */
 static void orc_wall_draw(uint32_t pid, uint64_t step, uint32_t stream, uint64_t seed, double theta_w,
@@ -640,6 +652,31 @@ static void orc_wall_draw(uint32_t pid, uint64_t step, uint32_t stream, uint64_t
     *t2 = st * r * sin(2.0 * ORC_PI * u[2]);
 }
 
+static void orc_reinsert(uint32_t pid, uint64_t step, uint64_t seed, const double *w0, float xmin, float xmax, float ymin,
+                         float ymax, float Ly, float pen, int two_d, float *xp, float *yp, double v[3])
+{
+    double th = w0[1], U = w0[2], sg = sqrt(th), mu = 0.5 * (U + sqrt(U * U + 4.0 * th)), vn = mu, u[4];
+    for (uint32_t a = 0; a < 8; ++a) {
+        orc_uniforms(pid, step, 16u + a, seed, u);
+        double c = mu + sg * sqrt(-2.0 * log(u[0])) * cos(2.0 * ORC_PI * u[1]);
+        if (c > 0.0 && (c / mu) * exp(1.0 - c / mu) >= u[2]) { vn = c; break; }
+    }
+    orc_uniforms(pid, step, 32u, seed, u);
+    double r = sg * sqrt(-2.0 * log(u[0]));
+    v[0] = vn; v[1] = w0[3] + r * cos(2.0 * ORC_PI * u[1]); v[2] = w0[4] + r * sin(2.0 * ORC_PI * u[1]);
+    float u2f = (float)u[2], u3f = (float)u[3];          /* (k + 1/2) 2^-23: exact in fp32 */
+    float xn = xmin + u3f * pen;
+    if (xn < xmin) xn = xmin;
+    if (xn >= xmax) xn = nextafterf(xmax, -INFINITY);
+    *xp = xn;
+    if (two_d) {
+        float yn = fmaf(u2f, Ly, ymin);
+        if (yn < ymin) yn = ymin;
+        if (yn >= ymax) yn = nextafterf(ymax, -INFINITY);
+        *yp = yn;
+    }
+}
+
 void orc_stream_walls(int64_t np, float *x, float *y, float *vx, float *vy, float *vz, const uint32_t *pid,
                       int32_t nx, int32_t ny, float x0, float y0, float dx, float dy, float dt,
                       const double *wall /* 4 x 5 */, int32_t body_kind, float bcx, float bcy, float bR,
@@ -647,11 +684,12 @@ void orc_stream_walls(int64_t np, float *x, float *y, float *vx, float *vy, floa
 {
     float xmin = x0, xmax = x0 + (float)nx * dx, ymin = y0, ymax = y0 + (float)ny * dy;
     float Lx = xmax - xmin, Ly = ymax - ymin;
+    float pen = (float)wall[2] * dt;                       /* fp32: fl(U_inf,x) * dt, one rounding */
 #pragma omp parallel for schedule(static)
     for (int64_t p = 0; p < np; ++p) {
         float xp = fmaf(vx[p], dt, x[p]), yp = fmaf(vy[p], dt, y[p]);
         double v[3] = {vx[p], vy[p], vz[p]};
-        int redrawn = 0;
+        int redrawn = 0, reinserted = 0;
         /* x pair */
         {
             int side = (xp < xmin) ? 0 : ((xp >= xmax) ? 1 : -1);
@@ -670,11 +708,14 @@ void orc_stream_walls(int64_t np, float *x, float *y, float *vx, float *vy, floa
                     xp = side ? xp - Lx : xp + Lx;
                     if (xp < xmin) xp = xmin;
                     if (xp >= xmax) xp = nextafterf(xmax, -INFINITY);
+                } else if (kind == 3) {
+                    orc_reinsert(pid[p], step, seed, wall, xmin, xmax, ymin, ymax, Ly, pen, ny > 1, &xp, &yp, v);
+                    redrawn = 1; reinserted = 1;
                 }
             }
         }
         /* y pair */
-        if (ny > 1) {
+        if (ny > 1 && !reinserted) {
             int side = (yp < ymin) ? 0 : ((yp >= ymax) ? 1 : -1);
             if (side >= 0) {
                 const double *w = wall + 5 * (2 + side);
@@ -691,6 +732,9 @@ void orc_stream_walls(int64_t np, float *x, float *y, float *vx, float *vy, floa
                     yp = side ? yp - Ly : yp + Ly;
                     if (yp < ymin) yp = ymin;
                     if (yp >= ymax) yp = nextafterf(ymax, -INFINITY);
+                } else if (kind == 3) {
+                    orc_reinsert(pid[p], step, seed, wall, xmin, xmax, ymin, ymax, Ly, pen, 1, &xp, &yp, v);
+                    redrawn = 1;
                 }
             }
         }

@@ -16,7 +16,7 @@ import math
 import numpy as np
 
 THETA_REF = 0.5
-WALL_NONE, WALL_DIFFUSE, WALL_PERIODIC = 0, 1, 2
+WALL_NONE, WALL_DIFFUSE, WALL_PERIODIC, WALL_INFLOW = 0, 1, 2, 3
 
 
 def tau_from_kn(kn, L=1.0):
@@ -195,7 +195,8 @@ def cylinder(nx=400, ny=300, seed=5, target=20_000_000, shuffle=False, kn_inf=0.
     counts = f["ppc"].reshape(-1)
     D = 2.0 * f["R"]
     tau_inf = tau_from_kn(kn_inf, D) / math.sqrt(2 * THETA_REF)   # c_mp = 1 at the freestream temperature
-    walls = [(WALL_NONE, 0.5, 0, 0, 0)] * 4
+    # outer faces: freestream reservoir (a particle that leaves re-enters at xmin from the Mach-10 freestream; reading R11)
+    walls = [(WALL_INFLOW, THETA_REF, 9.09, 0, 0)] * 4
     cfg = make_config(nx, ny, 1.0, 1.0, 0.055, tau_inf, walls, seed=seed, body=(f["cx"], f["cy"], f["R"], 1.25),
                       max_particles=int(counts.sum()))
     x, y, cell = _positions_in_cells(rng, counts, nx, ny, 1.0, 1.0)

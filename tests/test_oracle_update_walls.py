@@ -313,3 +313,56 @@ def test_couette_plate_reemission(orc, side):
     xe = np.float32(x0) + np.float32(-0.5 if side == 0 else 0.5)            # exact in fp32
     np.testing.assert_array_equal(out["x"], xw + (xw - xe))
     assert np.array_equal(out["y"], st["y"])                                # vy = 0: y untouched, ny = 1
+
+
+# ------------------------------------------------------------------------------------------------ S7: freestream reservoir
+def _flux_maxwellian_moments(U, theta):
+    """E[v], E[v^2] and the CDF of f(v) ~ v exp(-(v - U)^2 / (2 theta)) on v > 0 by plain quadrature (no sampler involved)."""
+    sg = math.sqrt(theta)
+    v = np.linspace(0.0, max(U, 0.0) + 12.0 * sg, 400001)
+    f = v * np.exp(-(v - U) ** 2 / (2.0 * theta))
+    dv = v[1] - v[0]
+    Z = f.sum() * dv
+    cdf = np.cumsum(f) * dv / Z
+    return (f * v).sum() * dv / Z, (f * v * v).sum() * dv / Z, v, cdf
+
+
+@pytest.mark.parametrize("U", [0.25, 9.09])
+def test_reservoir_reinsertion(orc, U):
+    """Reading R11: a particle leaving through a freestream face re-enters at xmin with the flux-
+    weighted drifting half-Maxwellian in v_x (moments and CDF against quadrature), Gaussian tangentials about U_inf, a
+    position uniform along the face and within one freestream step of it; the particle count is constant and every particle
+    ends inside the domain.  Subsonic (many rejections) and Mach 10 (almost none)."""
+    n, th = 200_000, 0.5
+    walls = [(wl.WALL_INFLOW, th, U, -0.2, 0.1)] * 4
+    cfg = wl.make_config(10, 8, 1.0, 0.5, 0.1, 1.0, walls, seed=23)
+    rng = np.random.default_rng(3)
+    # a quarter of the particles leaves through each face
+    q = n // 4
+    x = np.concatenate([np.full(q, 0.01), np.full(q, 9.99), rng.uniform(1, 9, q), rng.uniform(1, 9, q)]).astype(np.float32)
+    y = np.concatenate([rng.uniform(0.5, 3.5, q), rng.uniform(0.5, 3.5, q), np.full(q, 0.01), np.full(q, 3.99)]).astype(np.float32)
+    vx = np.concatenate([np.full(q, -1.0), np.full(q, 1.0), np.zeros(q), np.zeros(q)]).astype(np.float32)
+    vy = np.concatenate([np.zeros(q), np.zeros(q), np.full(q, -1.0), np.full(q, 1.0)]).astype(np.float32)
+    st = dict(x=x, y=y, vx=vx, vy=vy, vz=np.full(n, 7.0, np.float32), pid=np.arange(n, dtype=np.uint32))
+    out = orc.stream_walls(st, cfg, step=4)
+    assert out["x"].shape[0] == n and np.array_equal(out["pid"], st["pid"])
+    pen = float(np.float32(np.float32(U) * np.float32(cfg["dt"])))
+    assert out["x"].min() >= 0.0 and out["x"].max() <= pen * (1 + 1e-6) + 1e-7          # within one freestream step of xmin
+    assert out["y"].min() >= 0.0 and out["y"].max() < 4.0
+    se = 5 / math.sqrt(n)
+    m1, m2, vg, cdf = _flux_maxwellian_moments(U, th)
+    v = out["vx"].astype(np.float64)
+    assert np.all(v > 0)
+    assert abs(v.mean() - m1) < se * math.sqrt(m2 - m1 * m1) and abs((v * v).mean() - m2) < se * 3 * m2
+    for qq in (0.01, 0.1, 0.5, 0.9, 0.99):                                              # CDF at five quantiles
+        vq = vg[np.searchsorted(cdf, qq)]
+        assert abs((v <= vq).mean() - qq) < se
+    assert abs(out["vy"].mean() + 0.2) < se * math.sqrt(th) and abs(out["vz"].mean() - 0.1) < se * math.sqrt(th)
+    assert abs(out["vy"].var() - th) < se * 2 * th and abs(out["vz"].var() - th) < se * 2 * th
+    # positions: uniform along the face, uniform in the entry strip, independent of the face the particle left through
+    assert abs(out["y"].mean() - 2.0) < se * 4 / math.sqrt(12) and abs(out["x"].mean() - pen / 2) < se * pen / math.sqrt(12) + 1e-7
+    assert abs(np.corrcoef(out["y"], v)[0, 1]) < se and abs(np.corrcoef(out["x"], v)[0, 1]) < se
+    # a particle that stays inside is not touched
+    st2 = dict(st, x=np.full(n, 5.0, np.float32), y=np.full(n, 2.0, np.float32))
+    out2 = orc.stream_walls(st2, cfg, step=4)
+    assert np.array_equal(out2["vz"], st["vz"]) and np.array_equal(out2["vx"], st["vx"])
