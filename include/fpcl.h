@@ -63,6 +63,9 @@ extern "C" {
 #define FP_WALL_NONE     0
 #define FP_WALL_DIFFUSE  1        /* diffuse isothermal re-emission                          */
 #define FP_WALL_PERIODIC 2
+#define FP_WALL_INFLOW   3        /* freestream reservoir (R11): a particle leaving through such a face re-enters
+                                     at xmin from the freestream wall[0].{theta_w; ux > 0, uy, uz} with the flux-weighted
+                                     half-Maxwellian in v_x; wall[0] must then be FP_WALL_INFLOW too; constant particle count */
 
 typedef struct fp_ctx fp_ctx;
 

@@ -37,7 +37,12 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
         (int64_t)q.nx * q.ny >= ((int64_t)1 << 27) || q.max_particles >= ((int64_t)1 << 31) ||
         !(q.tau > 0.f) || (q.conserve_mode != 0 && q.conserve_mode != 1))
         return FP_ERR_ARG;
-    for (int k = 0; k < 4; ++k) if (q.wall[k].kind < 0 || q.wall[k].kind > 2) return FP_ERR_ARG;
+    for (int k = 0; k < 4; ++k) {
+        if (q.wall[k].kind < 0 || q.wall[k].kind > 3) return FP_ERR_ARG;
+        // a freestream face re-inserts at xmin from wall[0]'s freestream, which must flow into the domain
+        if (q.wall[k].kind == FP_WALL_INFLOW && (q.wall[0].kind != FP_WALL_INFLOW || !(q.wall[0].ux > 0.f) || !(q.wall[0].theta_w > 0.f)))
+            return FP_ERR_ARG;
+    }
     fp_ctx* c = new (std::nothrow) fp_ctx();
     if (!c) return FP_ERR_STATE;
     c->err[0] = 0;

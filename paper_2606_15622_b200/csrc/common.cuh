@@ -65,7 +65,7 @@ struct fp_ctx {
     uint32_t *h_err = nullptr, *d_err = nullptr;
     uint32_t *d_errdev = nullptr;    // device-memory copy of the word for kernels that must not run on bad boundaries
     int       mom_occ[6] = {0, 0, 0, 0, 0, 0};       // resident CTAs per SM of moments_warp_kernel<2^k, *>
-    int       mlp_tc_occ = 0;
+    int       mlp_tc_occ = 0, sw_occ[2] = {0, 0};
     bool      mlp_attr_w5 = false, mlp_attr_wd = false;
     // test / measurement switches read from the environment once, at fp_create
     bool      env_mom_seg = false, env_mom_no_seg = false, env_upd_seg = false, env_upd_no_seg = false;

@@ -15,6 +15,7 @@ struct sw_params {
     int32_t body_kind;
     float bcx, bcy, bR, bR_out, bR2, body_theta_w;
     uint32_t k0, k1, step_lo, step_hi;
+    float in_mu, in_sg, in_pen;     // freestream reservoir: mode of the flux density, sqrt(theta_inf), fl(U_inf,x * dt)
 };
 
 // One wall draw (R7): normal component sqrt(-2 theta_w ln u0) into the gas, tangentials
@@ -32,17 +33,50 @@ __device__ __forceinline__ void sw_wall_draw(const sw_params& P, uint32_t pid, u
     t2 = r * s;
 }
 
+// Freestream reservoir (FP_WALL_INFLOW, R11): re-insertion at xmin.  v_x from f(v) ~ v exp(-(v-U)^2/(2 theta)),
+// v > 0, by acceptance-rejection about the mode mu (candidate mu + sigma z, accepted iff v > 0 and (v/mu) e^(1 - v/mu) >= u2;
+// attempt a uses the Philox stream 16 + a, a < 8; then v = mu); tangentials and the entry position from stream 32.  The
+// position follows a fixed fp32 sequence (it decides the cell index).
+__device__ __noinline__ void sw_reinsert(const sw_params& P, uint32_t pid, bool two_d, float& xp, float& yp, float& v0,
+                                         float& v1, float& v2)
+{
+    float vn = P.in_mu;
+    for (uint32_t a = 0; a < 8u; ++a) {
+        const uint4 w = fpd_philox4x32_10(pid, P.step_lo, P.step_hi, 16u + a, P.k0, P.k1);
+        float s, c;
+        sincospif(2.0f * fpd_uniform(w.y), &s, &c);
+        const float cand = fmaf(P.in_sg * sqrtf(-2.0f * logf(fpd_uniform(w.x))), c, P.in_mu);
+        const float q = cand / P.in_mu;
+        if (cand > 0.0f && q * expf(1.0f - q) >= fpd_uniform(w.z)) { vn = cand; break; }
+    }
+    const uint4 w = fpd_philox4x32_10(pid, P.step_lo, P.step_hi, 32u, P.k0, P.k1);
+    const float r = P.in_sg * sqrtf(-2.0f * logf(fpd_uniform(w.x)));
+    float s, c;
+    sincospif(2.0f * fpd_uniform(w.y), &s, &c);
+    v0 = vn; v1 = fmaf(r, c, P.wall[0].uy); v2 = fmaf(r, s, P.wall[0].uz);
+    float xn = __fadd_rn(P.xmin, __fmul_rn(fpd_uniform(w.w), P.in_pen));
+    if (xn < P.xmin) xn = P.xmin;
+    if (xn >= P.xmax) xn = P.xmax_in;
+    xp = xn;
+    if (two_d) {
+        float yn = fmaf(fpd_uniform(w.z), P.Ly, P.ymin);
+        if (yn < P.ymin) yn = P.ymin;
+        if (yn >= P.ymax) yn = P.ymax_in;
+        yp = yn;
+    }
+}
+
 // One particle: stream, walls, body, key.  pid is read only by particles that hit something.
 struct sw_moved { float x, y, v0, v1, v2; uint32_t key; bool redrawn; };
 
-template <bool WRITE_KEYS>
+template <bool WRITE_KEYS, bool INFLOW>
 __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float yin, float v0, float v1,
                                             const uint32_t* __restrict__ pid, int64_t p)
 {
         float v2 = 0.0f;                           // vz is only ever replaced, never read
         float xp = fmaf(v0, P.dt, xin);
         float yp = fmaf(v1, P.dt, yin);
-        bool redrawn = false;
+        bool redrawn = false, reinserted = false;
         // x pair
         {
             const int side = (xp < P.xmin) ? 0 : ((xp >= P.xmax) ? 1 : -1);
@@ -60,11 +94,14 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
                     xp = side ? __fsub_rn(xp, P.Lx) : __fadd_rn(xp, P.Lx);
                     if (xp < P.xmin) xp = P.xmin;
                     if (xp >= P.xmax) xp = P.xmax_in;
+                } else if (INFLOW && w.kind == FP_WALL_INFLOW) {
+                    sw_reinsert(P, pid[p], P.ny > 1, xp, yp, v0, v1, v2);
+                    redrawn = true; reinserted = true;
                 }
             }
         }
         // y pair
-        if (P.ny > 1) {
+        if (P.ny > 1 && !reinserted) {
             const int side = (yp < P.ymin) ? 0 : ((yp >= P.ymax) ? 1 : -1);
             if (side >= 0) {
                 const fp_wall w = P.wall[2 + side];
@@ -80,6 +117,9 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
                     yp = side ? __fsub_rn(yp, P.Ly) : __fadd_rn(yp, P.Ly);
                     if (yp < P.ymin) yp = P.ymin;
                     if (yp >= P.ymax) yp = P.ymax_in;
+                } else if (INFLOW && w.kind == FP_WALL_INFLOW) {
+                    sw_reinsert(P, pid[p], true, xp, yp, v0, v1, v2);
+                    redrawn = true;
                 }
             }
         }
@@ -123,7 +163,8 @@ __device__ __forceinline__ void sw_hist(uint32_t* __restrict__ tile_hist, int nt
 
 // One particle per thread, grid-stride.  (Four particles per thread with 128-bit accesses was measured slower:
 // 37 vs 33 us at 4M particles.)
-template <bool WRITE_KEYS>
+// INFLOW: the grid has freestream faces (the re-insertion's call and registers stay out of the other instantiation).
+template <bool WRITE_KEYS, bool INFLOW>
 __global__ void __launch_bounds__(256)
 sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
           float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
@@ -139,7 +180,7 @@ sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __res
         const bool valid = p < np;
         uint32_t key = 0u;
         if (valid) {
-            const sw_moved m = sw_move<WRITE_KEYS>(P, x[p], y[p], vx[p], vy[p], pid, p);
+            const sw_moved m = sw_move<WRITE_KEYS, INFLOW>(P, x[p], y[p], vx[p], vy[p], pid, p);
             x[p] = m.x; y[p] = m.y; key = m.key;
             if (m.redrawn) { vx[p] = m.v0; vy[p] = m.v1; vz[p] = m.v2; }
             if (WRITE_KEYS) keys[p] = key;
@@ -153,6 +194,7 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
 {
     if (np == 0) return FP_OK;
     const fp_params& q = ctx->p;
+    const bool inflow = q.wall[0].kind == FP_WALL_INFLOW;      // fp_create: any freestream face implies wall[0] is one
     sw_params P;
     P.nx = q.nx; P.ny = q.ny; P.x0 = q.x0; P.y0 = q.y0; P.inv_dx = ctx->inv_dx; P.inv_dy = ctx->inv_dy; P.dt = q.dt;
     P.xmin = ctx->xmin; P.xmax = ctx->xmax; P.ymin = ctx->ymin; P.ymax = ctx->ymax;
@@ -164,14 +206,21 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
         volatile float r2 = q.body_R * q.body_R;    P.bR2 = r2;
     }
     P.body_theta_w = q.body_theta_w;
+    {   // freestream reservoir constants (only read when a face is FP_WALL_INFLOW)
+        const double U = q.wall[0].ux, th = q.wall[0].theta_w > 0.f ? q.wall[0].theta_w : 1.0;
+        P.in_mu = (float)(0.5 * (U + sqrt(U * U + 4.0 * th)));
+        P.in_sg = (float)sqrt(th);
+        volatile float pen = q.wall[0].ux * q.dt; P.in_pen = pen;
+    }
     P.k0 = (uint32_t)q.seed; P.k1 = (uint32_t)(q.seed >> 32);
     P.step_lo = (uint32_t)step; P.step_hi = (uint32_t)(step >> 32);
     const int threads = 256;
     const int64_t want = (np + threads - 1) / threads;
     // one resident wave of grid-striding CTAs (a partial extra wave costs up to 8 us at 4M particles)
-    static int socc = 0;
+    int& socc = ctx->sw_occ[inflow ? 1 : 0];
     if (socc == 0) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&socc, sw_kernel<true>, threads, 0);
+        if (inflow) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&socc, sw_kernel<true, true>, threads, 0);
+        else        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&socc, sw_kernel<true, false>, threads, 0);
         if (socc < 1) socc = 1;
     }
     const int64_t cap = (int64_t)ctx->num_sms * socc;
@@ -184,9 +233,11 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
             ctx->hist0_clean = false;
         }
         const uint32_t dmask = (1u << fpi_sort_digit_bits(ctx)) - 1u;
-        fp_launch(sw_kernel<true>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, keys_out, th, fp_div_up(np, SORT_TILE), dmask, P);
+        if (inflow) fp_launch(sw_kernel<true, true>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, keys_out, th, fp_div_up(np, SORT_TILE), dmask, P);
+        else        fp_launch(sw_kernel<true, false>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, keys_out, th, fp_div_up(np, SORT_TILE), dmask, P);
     } else {
-        fp_launch(sw_kernel<false>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
+        if (inflow) fp_launch(sw_kernel<false, true>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
+        else        fp_launch(sw_kernel<false, false>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
     }
     FP_LAUNCH_OK(ctx);
     FP_COUNT(ctx, 1);

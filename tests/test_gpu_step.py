@@ -90,7 +90,7 @@ def _cyl_small(wl):
     return cfg, st, tau_cell
 
 
-@pytest.mark.parametrize("name", ["couette", "cavity", "periodic", "cylinder"])
+@pytest.mark.parametrize("name", ["couette", "cavity", "periodic", "cylinder", "reservoir_subsonic"])
 def test_stream_walls(gpu, wl, orc, name):
     if name == "couette":
         cfg, st = wl.couette()
@@ -102,8 +102,14 @@ def test_stream_walls(gpu, wl, orc, name):
         w = [(wl.WALL_PERIODIC, 0.5, 0, 0, 0)] * 2 + [(wl.WALL_DIFFUSE, 0.7, 0.1, 0, 0.2), (wl.WALL_NONE, 0.5, 0, 0, 0)]
         cfg, st = wl.ragged(nx=20, ny=10, seed=2, mean_ppc=30.0, walls=w)
         cfg = dict(cfg, dt=float(np.float32(0.05)))
+    elif name == "reservoir_subsonic":
+        # freestream faces at U_inf = 0.25 sqrt(theta)-ish: the acceptance-rejection of the re-insertion rejects often, so
+        # the accept / reject decisions of the two sides (fp32 kernel, fp64 oracle) are compared on thousands of draws
+        w = [(wl.WALL_INFLOW, 0.5, 0.25, -0.2, 0.1)] * 4
+        cfg, st = wl.ragged(nx=20, ny=10, seed=4, mean_ppc=60.0, walls=w)
+        cfg = dict(cfg, dt=float(np.float32(0.08)))
     else:
-        cfg, st, _ = _cyl_small(wl)
+        cfg, st, _ = _cyl_small(wl)                      # Mach-10 freestream faces + the body
         cfg = dict(cfg, dt=float(np.float32(0.4)))
     cfg = dict(cfg, dt=float(np.float32(cfg["dt"])))
     step = 7
