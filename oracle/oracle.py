@@ -20,10 +20,17 @@ _lib = None
 
 
 def build(force=False):
-    """Compile fp_oracle.c with gcc (-O2 -ffp-contract=off so fp32 position arithmetic is not fused)."""
+    """Compile fp_oracle.c with gcc (-O2 -ffp-contract=off so fp32 position arithmetic is not fused).
+    ORACLE_SANITIZE=1 in the environment builds and loads an AddressSanitizer + UndefinedBehaviorSanitizer variant instead
+    (run the CPU pins with LD_PRELOAD=$(gcc -print-file-name=libasan.so); summary under profiles/)."""
+    global _LIB
+    san = os.environ.get("ORACLE_SANITIZE") == "1"
+    if san:
+        _LIB = os.path.join(_HERE, "libfp_oracle_asan.so")
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".%d.tmp" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-fopenmp", "-shared",
+        extra = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-g", "-O1"] if san else ["-O2"]
+        subprocess.check_call(["gcc"] + extra + ["-ffp-contract=off", "-fno-fast-math", "-std=c11", "-fopenmp", "-shared",
                                "-fPIC", "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
