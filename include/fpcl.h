@@ -214,6 +214,41 @@ int fp_step(fp_ctx* ctx, int64_t np,
             int32_t tau_mode, float tau_ref_n, float* tau_cell /* nullable unless tau_mode 1 */,
             uint64_t step, double* mom, float* coef, uint32_t* flags, int32_t* cell_start, void* stream);
 
+/* one domain cut into slabs of whole rows, one particle exchange per step (the paper itself runs one
+ * GPU, and independent replicas, :668).  Every slab's context is created with the GLOBAL fp_params (walls,
+ * body and the cell-index formula are the whole domain's; max_particles bounds what the slab may hold) and then told its
+ * rows: fp_set_slab(ctx, row0, nrows), before any other call; from then on the context has nx*nrows cells, numbered from its
+ * first row, and every per-cell array is that long.  A step on a slab: fp_stream_walls -> fp_slab_partition -> exchange
+ * (caller: device copies or NCCL) -> fp_collide.
+ * fp_slab_partition: stable partition of np particles by destination slab.  h_row_bounds [nslabs+1] (HOST) are the first
+ * rows of the slabs, from 0 to ny, 1 <= nslabs <= 64; slab_start [nslabs+1] (DEVICE) receives the offsets: particles
+ * slab_start[s] .. slab_start[s+1]-1 of the *_out arrays go to slab s, in input order.  Outputs may not alias inputs.
+ * If every receiver concatenates what it gets in ascending source-slab order (its own stayers in their place), fp_collide
+ * sees exactly the sub-sequence of the uncut domain's array that the slab owns, and the cut run is bit-identical to the
+ * uncut one (tests/test_gpu_slab.py).
+ * fp_collide: the part of fp_step after the move -- sort by cell, moments, closure, update -- with fp_step's arguments;
+ * positions are read only. */
+int fp_set_slab(fp_ctx* ctx, int32_t row0, int32_t nrows);
+/* on != 0: every per-cell result depends only on the cell's own particles in their array order, not on WHERE in the arrays
+ * they sit.  By default the moment gather starts each cell at the particle whose shared-memory bank suits the warp (no bank
+ * conflicts, ~4 us at 4M particles), which makes the fp32 summation order -- not the result beyond rounding -- depend on the
+ * cell's offset.  Switch it on (on every slab and on the uncut run) to compare decompositions bit for bit.  What stays
+ * context-dependent: the lanes-per-cell width G is chosen from the context's mean particles per cell (thresholds 56/112/224),
+ * and a warp's chunk of 32/G cells, counted from the slab's first cell, that overflows the 512-particle staging buffer is
+ * walked by the whole warp in another order.  Slabs whose mean density falls on the other side of a threshold, or whose
+ * chunks overflow where the uncut run's do not, agree with the uncut run to rounding only. */
+int fp_set_reproducible(fp_ctx* ctx, int32_t on);
+int fp_slab_partition(fp_ctx* ctx, int64_t np,
+                      const float* x, const float* y, const float* vx, const float* vy, const float* vz, const uint32_t* pid,
+                      float* x_out, float* y_out, float* vx_out, float* vy_out, float* vz_out, uint32_t* pid_out,
+                      const int32_t* h_row_bounds, int32_t nslabs, int32_t* slab_start, void* stream);
+int fp_collide(fp_ctx* ctx, int64_t np,
+               const float* x_a, const float* y_a, const float* vx_a, const float* vy_a, const float* vz_a, const uint32_t* pid_a,
+               float* x_b, float* y_b, float* vx_b, float* vy_b, float* vz_b, uint32_t* pid_b,
+               int32_t closure, const fp_mlp* h_mlp, float relax_w,
+               int32_t tau_mode, float tau_ref_n, float* tau_cell /* nullable unless tau_mode 1 */,
+               uint64_t step, double* mom, float* coef, uint32_t* flags, int32_t* cell_start, void* stream);
+
 /* Host-buffer convenience used by the end-to-end measurement: uploads the six SoA arrays from host memory
  * (pinned or pageable), runs fp_step on internally held device buffers sized max_particles, and downloads the
  * updated SoA plus cell_start, flags and coef back into the host arrays.  All uploads run on the caller's stream

@@ -52,6 +52,7 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
     c->env_mom_seg = getenv("FPCL_MOM_SEG") != nullptr; c->env_mom_no_seg = getenv("FPCL_MOM_NO_SEG") != nullptr;
     c->env_upd_seg = getenv("FPCL_UPD_SEG") != nullptr; c->env_upd_no_seg = getenv("FPCL_UPD_NO_SEG") != nullptr;
     c->ncell = q.nx * q.ny;
+    c->slab_row0 = 0; c->slab_rows = q.ny;
     int bits = 0;
     while (((int64_t)1 << bits) < (int64_t)c->ncell) ++bits;
     c->key_bits = bits;
@@ -117,6 +118,34 @@ int fpi_tau_from_counts(fp_ctx* ctx, const int32_t* cell_start, float tau_ref_n,
     return FP_OK;
 }
 
+// moments -> closure -> update on cell-sorted particles (the part of Algorithm 1/2 after the sort); shared by fp_step
+// and fp_collide
+static int fpi_after_sort(fp_ctx* ctx, int64_t np, float* vx_b, float* vy_b, float* vz_b, const uint32_t* pid_b, int32_t closure,
+                          const fp_mlp* h_mlp, float relax_w, int32_t tau_mode, float tau_ref_n, float* tau_cell, uint64_t step,
+                          double* mom, float* coef, uint32_t* flags, int32_t* cell_start, cudaStream_t st)
+{
+    int rc;
+    const float* tau_use = nullptr;
+    if (tau_mode == 1) {
+        if ((rc = fpi_tau_from_counts(ctx, cell_start, tau_ref_n, tau_cell, st)) != FP_OK) return rc;
+        tau_use = tau_cell;
+    }
+    // a3
+    const int32_t mode = closure == 0 ? 1 : 0;
+    const int32_t stride = mode ? 29 : 13;
+    if ((rc = fp_cell_moments(ctx, np, vx_b, vy_b, vz_b, cell_start, mode, mom, (void*)st)) != FP_OK) return rc;
+    fp_mark(ctx, 4, st);
+    // a4 | a5; the closure kernel also writes the per-cell constants of a6 (no separate prep launch)
+    if (closure == 0) rc = fpi_closure_exact(ctx, mom, tau_use, coef, flags, nullptr, true, st);
+    else              rc = fpi_closure_mlp(ctx, mom, stride, tau_use, h_mlp, relax_w, coef, flags, true, st);
+    if (rc != FP_OK) return rc;
+    fp_mark(ctx, 5, st);
+    // a6
+    rc = fpi_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, true, st);
+    fp_mark(ctx, 6, st);
+    return rc;
+}
+
 extern "C" int fp_step(fp_ctx* ctx, int64_t np,
                        float* x_a, float* y_a, float* vx_a, float* vy_a, float* vz_a, uint32_t* pid_a,
                        float* x_b, float* y_b, float* vx_b, float* vy_b, float* vz_b, uint32_t* pid_b,
@@ -145,25 +174,29 @@ extern "C" int fp_step(fp_ctx* ctx, int64_t np,
     if ((rc = fpi_sort_with_keys(ctx, np, ctx->key_b, true, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b,
                                  cell_start, nullptr, st)) != FP_OK) return rc;
     fp_mark(ctx, 3, st);
-    const float* tau_use = nullptr;
-    if (tau_mode == 1) {
-        if ((rc = fpi_tau_from_counts(ctx, cell_start, tau_ref_n, tau_cell, st)) != FP_OK) return rc;
-        tau_use = tau_cell;
-    }
-    // a3
-    const int32_t mode = closure == 0 ? 1 : 0;
-    const int32_t stride = mode ? 29 : 13;
-    if ((rc = fp_cell_moments(ctx, np, vx_b, vy_b, vz_b, cell_start, mode, mom, stream)) != FP_OK) return rc;
-    fp_mark(ctx, 4, st);
-    // a4 | a5; the closure kernel also writes the per-cell constants of a6 (no separate prep launch)
-    if (closure == 0) rc = fpi_closure_exact(ctx, mom, tau_use, coef, flags, nullptr, true, st);
-    else              rc = fpi_closure_mlp(ctx, mom, stride, tau_use, h_mlp, relax_w, coef, flags, true, st);
+    return fpi_after_sort(ctx, np, vx_b, vy_b, vz_b, pid_b, closure, h_mlp, relax_w, tau_mode, tau_ref_n, tau_cell, step, mom, coef,
+                          flags, cell_start, st);
+}
+
+// Algorithm 1/2 after the move: sort by cell -> moments -> closure -> update, on particles whose positions are final (a slab
+// after its exchange, or any caller that streams by itself).  Same arguments as fp_step.
+extern "C" int fp_collide(fp_ctx* ctx, int64_t np,
+                          const float* x_a, const float* y_a, const float* vx_a, const float* vy_a, const float* vz_a, const uint32_t* pid_a,
+                          float* x_b, float* y_b, float* vx_b, float* vy_b, float* vz_b, uint32_t* pid_b,
+                          int32_t closure, const fp_mlp* h_mlp, float relax_w,
+                          int32_t tau_mode, float tau_ref_n, float* tau_cell,
+                          uint64_t step, double* mom, float* coef, uint32_t* flags, int32_t* cell_start, void* stream)
+{
+    if (!ctx) return FP_ERR_ARG;
+    if (np < 0 || !mom || !coef || !flags || !cell_start || (closure != 0 && closure != 1) || (tau_mode != 0 && tau_mode != 1))
+        return fp_fail(ctx, FP_ERR_ARG, "fp_collide: bad argument");
+    if (closure == 1 && !h_mlp) return fp_fail(ctx, FP_ERR_ARG, "fp_collide: surrogate closure needs h_mlp");
+    if (tau_mode == 1 && !tau_cell) return fp_fail(ctx, FP_ERR_ARG, "fp_collide: tau_mode 1 needs tau_cell");
+    if (fp_state_check(ctx, "fp_collide") != FP_OK) return FP_ERR_STATE;
+    int rc = fp_sort_by_cell(ctx, np, x_a, y_a, vx_a, vy_a, vz_a, pid_a, x_b, y_b, vx_b, vy_b, vz_b, pid_b, cell_start, nullptr, stream);
     if (rc != FP_OK) return rc;
-    fp_mark(ctx, 5, st);
-    // a6
-    rc = fpi_velocity_update(ctx, np, vx_b, vy_b, vz_b, pid_b, cell_start, mom, stride, coef, tau_use, step, flags, true, st);
-    fp_mark(ctx, 6, st);
-    return rc;
+    return fpi_after_sort(ctx, np, vx_b, vy_b, vz_b, pid_b, closure, h_mlp, relax_w, tau_mode, tau_ref_n, tau_cell, step, mom, coef,
+                          flags, cell_start, (cudaStream_t)stream);
 }
 
 extern "C" uint64_t fp_launch_count(const fp_ctx* ctx) { return ctx ? ctx->launches : 0; }

@@ -50,6 +50,8 @@ struct fp_ctx {
     float     inv_dx = 0.f, inv_dy = 0.f;
     float     xmin = 0.f, xmax = 0.f, ymin = 0.f, ymax = 0.f, xmax_in = 0.f, ymax_in = 0.f, Lx = 0.f, Ly = 0.f;
     int       device = 0, num_sms = FPCL_NUM_SMS_DEFAULT;
+    bool      reproducible = false;  // fp_set_reproducible
+    int32_t   slab_row0 = 0, slab_rows = 0;   // fp_set_slab: this context owns rows row0 .. row0 + rows - 1 (rows = ny by default)
     // sort scratch (sized for max_particles)
     uint32_t *key_a = nullptr, *key_b = nullptr, *idx_a = nullptr, *idx_b = nullptr;
     uint32_t *block_hist = nullptr;  // two tables [bins][nblocks]: even passes use the first, odd passes the second
@@ -65,7 +67,7 @@ struct fp_ctx {
     uint32_t *h_err = nullptr, *d_err = nullptr;
     uint32_t *d_errdev = nullptr;    // device-memory copy of the word for kernels that must not run on bad boundaries
     int       mom_occ[6] = {0, 0, 0, 0, 0, 0};       // resident CTAs per SM of moments_warp_kernel<2^k, *>
-    int       mlp_tc_occ = 0, sw_occ[2] = {0, 0};
+    int       mlp_tc_occ = 0, sw_occ[2] = {0, 0}, gather_occ = 0;
     bool      mlp_attr_w5 = false, mlp_attr_wd = false;
     // test / measurement switches read from the environment once, at fp_create
     bool      env_mom_seg = false, env_mom_no_seg = false, env_upd_seg = false, env_upd_no_seg = false;
@@ -159,6 +161,7 @@ __device__ __forceinline__ void fpd_pdl()
 
 static inline int fp_div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
+
 // internal entry points shared between translation units (not exported)
 int fpi_sort_digit_bits(const fp_ctx* ctx);           // width of one radix digit for this grid
 int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0_ready,
@@ -188,6 +191,29 @@ __device__ __forceinline__ int32_t fpd_axis_index(float p, float p0, float inv_d
     if (!(t >= 0.0f)) return 0;
     if (t >= (float)n) return n - 1;
     return (int32_t)t;
+}
+
+// Cell key of a position.  A context that is a slab of the grid (fp_set_slab: rows row0 .. row0 + nrows - 1) numbers its
+// cells from its first row; the row itself always comes from the GLOBAL formula, so that a particle gets the same cell
+// whether the grid is cut or not.  (nrows = ny, row0 = 0 without a slab.)
+struct fp_grid { int32_t nx, ny; float x0, y0, inv_dx, inv_dy; int32_t row0, nrows; };
+__device__ __forceinline__ int32_t fpd_cell_key(float x, float y, const fp_grid& g)
+{
+    const int32_t ix = fpd_axis_index(x, g.x0, g.inv_dx, g.nx);
+    int32_t iy = 0;
+    if (g.ny > 1) {
+        iy = fpd_axis_index(y, g.y0, g.inv_dy, g.ny) - g.row0;
+        iy = min(max(iy, 0), g.nrows - 1);                 // rows of other slabs: only if the caller skipped the exchange
+    }
+    return iy * g.nx + ix;
+}
+
+static inline fp_grid fp_grid_of(const fp_ctx* ctx)
+{
+    fp_grid g;
+    g.nx = ctx->p.nx; g.ny = ctx->p.ny; g.x0 = ctx->p.x0; g.y0 = ctx->p.y0; g.inv_dx = ctx->inv_dx; g.inv_dy = ctx->inv_dy;
+    g.row0 = ctx->slab_row0; g.nrows = ctx->slab_rows;
+    return g;
 }
 
 // Philox4x32-10 (Salmon et al., SC'11; R6).  counter (c0..c3), key (k0,k1).

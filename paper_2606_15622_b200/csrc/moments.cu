@@ -175,7 +175,8 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
 #endif
 template <int G, bool FULL, class Hook>
 __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,
-                                             bool have, int gl, int group, double* __restrict__ rec, Hook after_reads)
+                                             bool have, int gl, int group, double* __restrict__ rec, bool norot,
+                                             Hook after_reads)
 {
     constexpr int NP = (FULL || G > 16) ? 32 : 16;
     constexpr int NREC = FULL ? 29 : 13;
@@ -187,7 +188,7 @@ __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, c
     if (n > 0) { px = x[0]; py = y[0]; pz = z[0]; }
     const float2 npx = fpd_dup(-px), npy = fpd_dup(-py), npz = fpd_dup(-pz);
     // rotation: particle o of the cell sits in bank G*group
-    int32_t o = (int32_t)((uint32_t)(G * group) - (fpt_smem_u32(x) >> 2)) & 31;
+    int32_t o = norot ? 0 : (int32_t)((uint32_t)(G * group) - (fpt_smem_u32(x) >> 2)) & 31;
     while (n > 0 && o >= n) o -= n;
     if (n <= 0) o = 0;
     const int32_t full = n / (2 * G);                       // steps in which all 2G particles exist
@@ -409,7 +410,7 @@ __device__ __noinline__ void mom_dense_chunk(const float* __restrict__ vx, const
         const int64_t cellc = chunk * cpw + c;
         if (cellc >= ncell) continue;                                             // warp-uniform
         double* recc = mom + (size_t)cellc * NREC;
-        const fpw_range rc = fpw_range_of(s1c, e1c, np, aligned != 0, MOM_CAP);
+        const fpw_range rc = fpw_range_of(s1c, e1c, np, (aligned & 1) != 0, MOM_CAP);
         if (rc.staged) {
             fpt_fence_proxy_async();                 // earlier generic writes to the buffer vs the new bulk copy
             __syncwarp();
@@ -483,7 +484,7 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
         return fpd_cells_ok(v, c * CPW, cells, ncell, np, lane, err) ? v : 0;
     };
     auto range_of = [&](int32_t cs) {
-        return fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, aligned != 0, MOM_CAP);
+        return fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, (aligned & 1) != 0, MOM_CAP);
     };
     auto issue = [&](const fpw_range& r, int b) {
         const uint32_t bytes = (uint32_t)r.nb * 4u;
@@ -543,7 +544,7 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
                     }
                     reissued = true;
                 };
-                mom_cell_rot<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, sb, n, have, gl, group, rec, hook);
+                mom_cell_rot<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, sb, n, have, gl, group, rec, (aligned & 2) != 0, hook);
             } else if (NST == 1) {
                 auto hook = [&]() {
                     if (more) {
@@ -581,7 +582,8 @@ static void launch_moments(fp_ctx* ctx, int64_t np, const float* vx, const float
                            const int32_t* cell_start, int32_t mode, double* mom, cudaStream_t st)
 {
     const int cells_per_block = MOM_WARPS * (32 / G);
-    const int aligned = ((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0 ? 1 : 0;
+    // bit 0: 16-byte aligned arrays (bulk copies); bit 1: fp_set_reproducible (no address-dependent visiting order)
+    const int aligned = (((((uintptr_t)vx) | ((uintptr_t)vy) | ((uintptr_t)vz)) & 15u) == 0 ? 1 : 0) | (ctx->reproducible ? 2 : 0);
     const size_t smem = (size_t)MOM_WARPS * MOM_STAGES * 3 * MOM_CAP * sizeof(float) + MOM_WARPS * 2 * sizeof(uint64_t);
     int& occ = ctx->mom_occ[G == 2 ? 0 : G == 4 ? 1 : G == 8 ? 2 : G == 16 ? 3 : 4];   // resident CTAs per SM
     if (occ == 0) {

@@ -15,8 +15,7 @@
 // cell keys of tile blockIdx.x plus the tile's histogram of the first radix digit
 __global__ void __launch_bounds__(SORT_THREADS)
 key_kernel(int64_t np, const float* __restrict__ x, const float* __restrict__ y, uint32_t* __restrict__ keys,
-           int32_t nx, int32_t ny, float x0, float y0, float inv_dx, float inv_dy,
-           uint32_t* __restrict__ block_hist, int nblocks, int bins)
+           const fp_grid G, uint32_t* __restrict__ block_hist, int nblocks, int bins)
 {
     __shared__ uint32_t h[SORT_MAX_BINS];
     for (int b = threadIdx.x; b < bins; b += SORT_THREADS) h[b] = 0;
@@ -29,9 +28,7 @@ key_kernel(int64_t np, const float* __restrict__ x, const float* __restrict__ y,
         const bool valid = p < np;
         uint32_t key = 0;
         if (valid) {
-            const int32_t ix = fpd_axis_index(x[p], x0, inv_dx, nx);
-            const int32_t iy = (ny > 1) ? fpd_axis_index(y[p], y0, inv_dy, ny) : 0;
-            key = (uint32_t)(iy * nx + ix);
+            key = (uint32_t)fpd_cell_key(x[p], y[p], G);
             keys[p] = key;
         }
         if (valid) atomicAdd(&h[key & mask], 1u);
@@ -231,7 +228,7 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
 // FROM_POS (packed sort): the sorted keys were not stored; a particle's key is recomputed from the positions this
 // kernel gathers anyway (the same function of the same numbers as the key that was sorted), the left neighbour's
 // key comes from the lane below or, for lane 0, from the neighbour's positions.
-struct gather_grid { int32_t nx, ny; float x0, y0, inv_dx, inv_dy; };
+typedef fp_grid gather_grid;
 
 template <bool FROM_POS>
 __global__ void __launch_bounds__(256)
@@ -258,9 +255,7 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
         if (valid) {
             px = x[s]; py = y[s];
             if (FROM_POS) {
-                const int32_t ix = fpd_axis_index(px, Gd.x0, Gd.inv_dx, Gd.nx);
-                const int32_t iy = (Gd.ny > 1) ? fpd_axis_index(py, Gd.y0, Gd.inv_dy, Gd.ny) : 0;
-                key = iy * Gd.nx + ix;
+                key = fpd_cell_key(px, py, Gd);
             } else {
                 key = (int)skeys[k];
                 lo = (k == 0) ? 0 : (int)skeys[k - 1] + 1;
@@ -270,9 +265,7 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
             int prev = __shfl_up_sync(0xffffffffu, key, 1);
             if (lane == 0 && k > 0 && valid) {
                 const uint32_t s2 = perm[k - 1];
-                const int32_t ix = fpd_axis_index(x[s2], Gd.x0, Gd.inv_dx, Gd.nx);
-                const int32_t iy = (Gd.ny > 1) ? fpd_axis_index(y[s2], Gd.y0, Gd.inv_dy, Gd.ny) : 0;
-                prev = iy * Gd.nx + ix;
+                prev = fpd_cell_key(x[s2], y[s2], Gd);
             }
             lo = (k == 0) ? 0 : prev + 1;
         }
@@ -351,7 +344,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     ctx->hist0_clean = (passes & 1) == 0;             // the last scan zeroed the table the last pass did not use
     fp_mark(ctx, 2, st);
     // one resident wave of grid-striding CTAs (a partial second wave costs 4 us at 4M particles)
-    static int gocc = 0;
+    int& gocc = ctx->gather_occ;
     if (gocc == 0) {
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&gocc, gather_kernel<true>, 256, 0);
         if (gocc < 1) gocc = 1;
@@ -359,8 +352,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     const int64_t cap = (int64_t)ctx->num_sms * gocc;
     const int64_t want = (np + 255) / 256;
     const int gblocks = (int)(want < cap ? want : cap);
-    gather_grid Gd;
-    Gd.nx = ctx->p.nx; Gd.ny = ctx->p.ny; Gd.x0 = ctx->p.x0; Gd.y0 = ctx->p.y0; Gd.inv_dx = ctx->inv_dx; Gd.inv_dy = ctx->inv_dy;
+    const gather_grid Gd = fp_grid_of(ctx);
     if (ctx->ev_before_gather) FP_CUDA_OK(ctx, cudaStreamWaitEvent(st, ctx->ev_before_gather, 0));
     if (packed)
         fp_launch(gather_kernel<true>, gblocks, 256, 0, st, np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
@@ -390,10 +382,9 @@ extern "C" int fp_sort_by_cell(fp_ctx* ctx, int64_t np,
         return fp_fail(ctx, FP_ERR_ARG, "fp_sort_by_cell: outputs may not alias inputs");
     cudaStream_t st = (cudaStream_t)stream;
     if (np > 0) {
-        const fp_params& q = ctx->p;
         const int nblocks = fp_div_up(np, SORT_TILE);
-        key_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, x, y, ctx->key_b, q.nx, q.ny, q.x0, q.y0, ctx->inv_dx, ctx->inv_dy,
-                                                    ctx->block_hist, nblocks, 1 << fpi_sort_digit_bits(ctx));
+        key_kernel<<<nblocks, SORT_THREADS, 0, st>>>(np, x, y, ctx->key_b, fp_grid_of(ctx), ctx->block_hist, nblocks,
+                                                    1 << fpi_sort_digit_bits(ctx));
         FP_LAUNCH_OK(ctx);
         FP_COUNT(ctx, 1);
     }

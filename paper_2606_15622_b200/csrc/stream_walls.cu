@@ -15,6 +15,7 @@ struct sw_params {
     int32_t body_kind;
     float bcx, bcy, bR, bR_out, bR2, body_theta_w;
     uint32_t k0, k1, step_lo, step_hi;
+    fp_grid grid;                    // cell keys (slab-aware)
     float in_mu, in_sg, in_pen;     // freestream reservoir: mode of the flux density, sqrt(theta_inf), fl(U_inf,x * dt)
 };
 
@@ -143,9 +144,7 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
         sw_moved m;
         m.x = xp; m.y = yp; m.v0 = v0; m.v1 = v1; m.v2 = v2; m.redrawn = redrawn; m.key = 0u;
         if (WRITE_KEYS) {
-            const int32_t ix = fpd_axis_index(xp, P.x0, P.inv_dx, P.nx);
-            const int32_t iy = (P.ny > 1) ? fpd_axis_index(yp, P.y0, P.inv_dy, P.ny) : 0;
-            m.key = (uint32_t)(iy * P.nx + ix);
+            m.key = (uint32_t)fpd_cell_key(xp, yp, P.grid);
         }
         return m;
 }
@@ -206,6 +205,7 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
         volatile float r2 = q.body_R * q.body_R;    P.bR2 = r2;
     }
     P.body_theta_w = q.body_theta_w;
+    P.grid = fp_grid_of(ctx);
     {   // freestream reservoir constants (only read when a face is FP_WALL_INFLOW)
         const double U = q.wall[0].ux, th = q.wall[0].theta_w > 0.f ? q.wall[0].theta_w : 1.0;
         P.in_mu = (float)(0.5 * (U + sqrt(U * U + 4.0 * th)));

@@ -101,7 +101,9 @@ __device__ __forceinline__ fpw_range fpw_range_of(int32_t s0, int32_t s1, int64_
     const int32_t np4 = (int32_t)(np & ~(int64_t)3);
     const int32_t end4 = min((s1 + 3) & ~3, np4);
     r.nb = max(end4 - r.a0, 0);
-    r.staged = aligned && s1 > s0 && (s1 - r.a0) <= cap;
+    // (s1 - a0) <= (s1 - s0) + 3: the bound does not depend on where the slice starts, so a chunk takes the same path
+    // (staged or walked) wherever its particles sit in the arrays (fp_set_reproducible, slab decompositions)
+    r.staged = aligned && s1 > s0 && (s1 - s0) + 3 <= cap;
     return r;
 }
 

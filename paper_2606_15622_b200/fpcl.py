@@ -20,7 +20,8 @@ FLAG_EMPTY, FLAG_LOWCOUNT, FLAG_SINGULAR, FLAG_ILLCOND, FLAG_ALPHA, FLAG_SKIPPED
 EXPORTS = ["fp_create", "fp_destroy", "fp_last_error", "fp_version", "fp_sort_by_cell", "fp_cell_moments",
            "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host",
            "fp_timing_enable", "fp_timing_read", "fp_launch_count", "fp_set_mlp_tensor_cores", "fp_cell_diagnostics",
-           "fp_average_results", "fp_cell_sixth_moment", "fp_reserve", "fp_check"]
+           "fp_average_results", "fp_cell_sixth_moment", "fp_reserve", "fp_check", "fp_set_slab", "fp_slab_partition",
+           "fp_collide", "fp_set_reproducible"]
 NSTAGES = 6
 STAGE_NAMES = ["stream_walls", "sort_keys", "gather", "moments", "closure", "update"]
 
@@ -83,6 +84,10 @@ def load(path=None):
     lib.fp_launch_count.argtypes = [vp]
     lib.fp_set_mlp_tensor_cores.argtypes = [vp, i32]
     lib.fp_reserve.argtypes = [vp, C.POINTER(FpMlp), i32]
+    lib.fp_set_slab.argtypes = [vp, i32, i32]
+    lib.fp_set_reproducible.argtypes = [vp, i32]
+    lib.fp_slab_partition.argtypes = [vp, i64] + [vp] * 12 + [C.POINTER(i32), i32, vp, vp]
+    lib.fp_collide.argtypes = [vp, i64] + [vp] * 12 + [i32, C.POINTER(FpMlp), f32, i32, f32, vp, u64, vp, vp, vp, vp, vp]
     lib.fp_check.argtypes = [vp, vp]
     for name in EXPORTS:
         if name not in ("fp_last_error", "fp_version", "fp_launch_count"):
@@ -220,6 +225,35 @@ def fp_step(ctx, np_, a, b, closure, mlp, relax_w, tau_mode, tau_ref_n, tau_cell
     _check(ctx, load().fp_step(ctx, np_, *args, closure, mp, relax_w, tau_mode, tau_ref_n, _ptr(tau_cell, f), step,
                                _ptr(mom, torch.float64), _ptr(coef, f), _ptr(flags, u), _ptr(cell_start, u),
                                _stream()), "fp_step")
+
+
+def fp_collide(ctx, np_, a, b, closure, mlp, relax_w, tau_mode, tau_ref_n, tau_cell, step, mom, coef, flags, cell_start):
+    """fp_step without the move: sort by cell -> moments -> closure -> update (positions of ``a`` are final)."""
+    f, u = torch.float32, torch.int32
+    args = [_ptr(a[k], f, np_) for k in ("x", "y", "vx", "vy", "vz")] + [_ptr(a["pid"], u, np_)]
+    args += [_ptr(b[k], f, np_) for k in ("x", "y", "vx", "vy", "vz")] + [_ptr(b["pid"], u, np_)]
+    mp = C.byref(mlp.c_struct) if mlp is not None else C.POINTER(FpMlp)()
+    _check(ctx, load().fp_collide(ctx, np_, *args, closure, mp, relax_w, tau_mode, tau_ref_n, _ptr(tau_cell, f), step,
+                                  _ptr(mom, torch.float64), _ptr(coef, f), _ptr(flags, u), _ptr(cell_start, u),
+                                  _stream()), "fp_collide")
+
+
+def fp_set_reproducible(ctx, on=True):
+    _check(ctx, load().fp_set_reproducible(ctx, int(bool(on))), "fp_set_reproducible")
+
+
+def fp_set_slab(ctx, row0, nrows):
+    _check(ctx, load().fp_set_slab(ctx, int(row0), int(nrows)), "fp_set_slab")
+
+
+def fp_slab_partition(ctx, np_, a, b, row_bounds, slab_start):
+    """Stable partition of a's particles by destination slab into b; slab_start [nslabs+1] int32 on the device."""
+    f, u = torch.float32, torch.int32
+    args = [_ptr(a[k], f, np_) for k in ("x", "y", "vx", "vy", "vz")] + [_ptr(a["pid"], u, np_)]
+    args += [_ptr(b[k], f, np_) for k in ("x", "y", "vx", "vy", "vz")] + [_ptr(b["pid"], u, np_)]
+    rb = (C.c_int32 * len(row_bounds))(*[int(r) for r in row_bounds])
+    _check(ctx, load().fp_slab_partition(ctx, np_, *args, rb, len(row_bounds) - 1, _ptr(slab_start, u), _stream()),
+           "fp_slab_partition")
 
 
 def _hptr(a, dtype):
