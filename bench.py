@@ -719,6 +719,15 @@ def main():
                                                          "frac": single["moments"]["frac_of_hbm_peak"]},
                              "dominant_kernel_in_step": {"kernel": dom, "ms": single[dom]["ms"],
                                                          "frac": single[dom]["frac_of_hbm_peak"]}}}
+        # the update kernel against its own bound ("What bounds it: the FMA pipe"): the pass-A loop
+        # needs 446 scheduler cycles per 64 particles (measured in isolation), a B200 has 148 x 4 schedulers
+        sm_hz = 1e6 * float(clocks.get("sm_mhz") or 1965.0)
+        sms = torch.cuda.get_device_properties(0).multi_processor_count
+        need = 446.0 / 64.0 * np_ / (cold["update"]["ms"] * 1e-3)
+        roofline["also"]["update_alu"] = {"bound": "alu", "unit": "scheduler-cycles/s", "achieved": need,
+                                          "peak": sms * 4 * sm_hz, "frac": need / (sms * 4 * sm_hz),
+                                          "peak_source": "SMs x 4 schedulers x SM clock under load",
+                                          "note": "pass A only: Philox4x32-10 + Box-Muller + cubic drift per particle"}
 
     extras = {}
     if rank == 0 and not args.no_extras:
