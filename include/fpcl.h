@@ -143,6 +143,29 @@ int fp_sort_by_cell(fp_ctx* ctx, int64_t np,
 int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const float* vy, const float* vz,
                     const int32_t* cell_start, int32_t mode, double* mom, void* stream);
 
+/* a3 without a context and WITHOUT ANY ALLOCATION -- for callers that may not call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  Same operation, arguments and record layout as
+ * fp_cell_moments (mode 0 = LITE, 1 = FULL), same fp32-sum / fp64-shift arithmetic as its
+ * slice path (moments_seg.cuh): results agree with fp_cell_moments within the moment tolerance (1e-6), not bit for bit.
+ * The entry point calls no cudaMalloc, cudaFree or allocating library routine; its only scratch (28 doubles per cell and
+ * a status word) is a file-scope __device__ array of FP_STATIC_MAX_CELLS x 28 doubles = 3.5 MiB that every GPU which
+ * loads the library holds until the process exits.
+ *   - ncell > FP_STATIC_MAX_CELLS, np outside [0, 2^31), mode not 0/1, a null pointer, or vx/vy/vz not 16-byte aligned:
+ *     FP_ERR_ARG, nothing launched; the reason is in fp_static_last_error() (thread-local text).
+ *   - every call SHARES the one array, which keeps the last call's contents: the call clears what it uses on `stream`
+ *     first, so calls in stream order are independent, but calls that overlap on the GPU (other streams, other threads)
+ *     race on it and give wrong records.
+ *   - cell_start is validated on the device as everywhere else; if it is not a sorted prefix ending at np, `mom` is left
+ *     untouched.  d_status (device pointer to one uint32, nullable) receives 0 or the state bits (1 = bad cell_start) in
+ *     stream order; there is no context to carry a sticky host-side state.
+ *   - the first call on a device resolves the array's device address (cudaGetSymbolAddress) with that device current:
+ *     make that call outside stream capture.  Asynchronous on `stream` like every other call. */
+#define FP_STATIC_MAX_CELLS 16384
+int fp_cell_moments_static(int64_t np, const float* vx, const float* vy, const float* vz,
+                           const int32_t* cell_start, int32_t ncell, int32_t mode, double* mom,
+                           uint32_t* d_status /* nullable */, void* stream);
+const char* fp_static_last_error(void);
+
 /* a4 -- exact cubic-FP closure: assemble and solve the 9x9 moment-matching system per cell (Eq. 10
  * :121, Table 1 :130-136; derivation DESIGN.md R2, scaling and flags R3).  tau_cell nullable (then params.tau).
  * coef [ncell*9] fp32, flags [ncell] (overwritten).  kappa_est nullable: if given receives the library's estimate of

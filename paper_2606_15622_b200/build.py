@@ -16,7 +16,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJDIR = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libfpcl.so")
 SOURCES = ["api.cu", "stream_walls.cu", "sort.cu", "moments.cu", "closure_exact.cu", "closure_mlp.cu", "update.cu",
-           "diagnostics.cu", "slab.cu"]
+           "diagnostics.cu", "slab.cu", "moments_static.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
          "-I", INCLUDE] + os.environ.get("FPCL_NVCC_FLAGS", "").split()

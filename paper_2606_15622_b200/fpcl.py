@@ -21,7 +21,8 @@ EXPORTS = ["fp_create", "fp_destroy", "fp_last_error", "fp_version", "fp_sort_by
            "fp_closure_exact", "fp_closure_mlp", "fp_velocity_update", "fp_stream_walls", "fp_step", "fp_step_host",
            "fp_timing_enable", "fp_timing_read", "fp_launch_count", "fp_set_mlp_tensor_cores", "fp_cell_diagnostics",
            "fp_average_results", "fp_cell_sixth_moment", "fp_reserve", "fp_check", "fp_set_slab", "fp_slab_partition",
-           "fp_collide", "fp_set_reproducible"]
+           "fp_collide", "fp_set_reproducible", "fp_cell_moments_static", "fp_static_last_error"]
+FP_STATIC_MAX_CELLS = 16384
 NSTAGES = 6
 STAGE_NAMES = ["stream_walls", "sort_keys", "gather", "moments", "closure", "update"]
 
@@ -90,9 +91,11 @@ def load(path=None):
     lib.fp_collide.argtypes = [vp, i64] + [vp] * 12 + [i32, C.POINTER(FpMlp), f32, i32, f32, vp, u64, vp, vp, vp, vp, vp]
     lib.fp_check.argtypes = [vp, vp]
     for name in EXPORTS:
-        if name not in ("fp_last_error", "fp_version", "fp_launch_count"):
+        if name not in ("fp_last_error", "fp_version", "fp_launch_count", "fp_static_last_error"):
             getattr(lib, name).restype = C.c_int
     lib.fp_launch_count.restype = C.c_uint64
+    lib.fp_cell_moments_static.argtypes = [i64, vp, vp, vp, vp, i32, i32, vp, vp, vp]
+    lib.fp_static_last_error.restype = C.c_char_p
     if path is None:
         _lib = lib
     return lib
@@ -170,6 +173,17 @@ def fp_cell_moments(ctx, np_, vx, vy, vz, cell_start, mode, mom):
     _check(ctx, load().fp_cell_moments(ctx, np_, _ptr(vx, f, np_), _ptr(vy, f, np_), _ptr(vz, f, np_),
                                        _ptr(cell_start, torch.int32), mode, _ptr(mom, torch.float64), _stream()),
            "fp_cell_moments")
+
+
+def fp_cell_moments_static(np_, vx, vy, vz, cell_start, ncell, mode, mom, d_status=None):
+    """The context-free, allocation-free moment gather (include/fpcl.h); marshalling only."""
+    f = torch.float32
+    lib = load()
+    rc = lib.fp_cell_moments_static(np_, _ptr(vx, f, np_), _ptr(vy, f, np_), _ptr(vz, f, np_),
+                                    _ptr(cell_start, torch.int32, ncell + 1), ncell, mode,
+                                    _ptr(mom, torch.float64, ncell * (29 if mode else 13)), _ptr(d_status, torch.int32), _stream())
+    if rc != 0:
+        raise FpclError("fp_cell_moments_static failed with code %d: %s" % (rc, lib.fp_static_last_error().decode()))
 
 
 def fp_closure_exact(ctx, mom_full, tau_cell, coef, flags, kappa_est=None):
