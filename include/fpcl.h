@@ -179,6 +179,10 @@ int fp_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell 
 
 /* a5 -- fused MLP surrogate: features -> standardise -> dense layers -> de-standardise (PAPER.md:264, :309,
  * :327).  mom_stride 13 or 29.  relax_w in (0,1]: coef <- w*new + (1-w)*old; 1 overwrites.
+ * With relax_w < 1 `coef` is read: it must hold the previous step's coefficients, or zeros before the first step (not
+ * uninitialised memory).  A cell whose nine old coefficients are all exactly zero -- it was EMPTY at the previous step,
+ * or the array was zero-initialised -- has no history and takes the new values unblended (R12); otherwise
+ * a newly populated cell would start at w times its coefficients, i.e. 1/w times too slow a relaxation.
  * The caller's weights (device memory, row-major [out][in]) are re-packed into context scratch by a small
  * kernel on every call, on the same stream: weights changed in place between calls are always picked up. */
 int fp_closure_mlp(fp_ctx* ctx, const double* mom, int32_t mom_stride, const float* tau_cell /* nullable */,

@@ -408,7 +408,8 @@ void orc_average_results(int64_t n, const double *x, int64_t k, double *avg)
  *   T = theta/theta_ref, pi_ij = n (P_ij - theta delta_ij), q_i = n h_i / 2  (R4; pi33 dropped as redundant).
  * feature_set 1 (paper's 16, definitions UNPINNED R4): rho=n, T, U(3), Pi_ij = n P_ij (6), q(3),
  *   DM2 = 3 theta, nu = 1/tau.
- * relax_w: coef <- w*new + (1-w)*old; w = 1 overwrites (old is not read).
+ * relax_w: coef <- w*new + (1-w)*old; w = 1 overwrites (old is not read); a cell whose old coefficients
+ * are all exactly zero (EMPTY at the previous step, zero-initialised first step) has no history and is not blended (R12).
  * Flags: EMPTY -> zeros; N < min_count or theta <= 0 -> Langevin, LOWCOUNT/SINGULAR; non-finite output ->
  * Langevin + NONFINITE.
  * ------------------------------------------------------------------------------------------------ */
@@ -482,8 +483,12 @@ void orc_closure_mlp(int32_t ncell, const double *mom, int32_t stride, const flo
             for (int k = 0; k < 9; ++k) if (!isfinite(y[k])) finite = 0;
             if (!finite) { orc_langevin(tau, y); flag = ORC_FLAG_NONFINITE; }
         }
+        /* reading R12: a cell without history -- all nine old coefficients exactly zero: it was EMPTY at the previous
+         * step, or this is the first step on a zero-initialised array -- takes the new values unblended */
+        int history = 0;
+        if (relax_w != 1.0) for (int k = 0; k < 9; ++k) if (coef_old[(size_t)c * 9 + k] != 0.0) history = 1;
         for (int k = 0; k < 9; ++k)
-            out[k] = (relax_w == 1.0) ? y[k] : relax_w * y[k] + (1.0 - relax_w) * coef_old[(size_t)c * 9 + k];
+            out[k] = history ? relax_w * y[k] + (1.0 - relax_w) * coef_old[(size_t)c * 9 + k] : y[k];
         flags[c] = flag;
     }
 }

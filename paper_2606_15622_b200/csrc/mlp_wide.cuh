@@ -348,8 +348,14 @@ mlp_wide_kernel(const double* __restrict__ mom, const float* __restrict__ tau_ce
                     y[0] = d; y[1] = 0.f; y[2] = 0.f; y[3] = d; y[4] = 0.f; y[5] = d; y[6] = 0.f; y[7] = 0.f; y[8] = 0.f;
                 }
                 if (P.relax_w != 1.0f) {
+                    // no history (all nine old coefficients zero: EMPTY last step / zero-initialised first step): no blend (R12)
+                    bool history = false;
 #pragma unroll
-                    for (int k = 0; k < 9; ++k) y[k] = P.relax_w * y[k] + (1.0f - P.relax_w) * out[k];
+                    for (int k = 0; k < 9; ++k) history = history || out[k] != 0.0f;
+                    if (history) {
+#pragma unroll
+                        for (int k = 0; k < 9; ++k) y[k] = P.relax_w * y[k] + (1.0f - P.relax_w) * out[k];
+                    }
                 }
             }
 #pragma unroll

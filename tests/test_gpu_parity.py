@@ -377,6 +377,7 @@ def test_closure_mlp(gpu, wl, orc, shape, stride):
       gpu.fp_set_mlp_tensor_cores(ctx.h, tc)
       for relax_w in (1.0, 0.2):
           old = np.random.default_rng(8).normal(size=(mom.shape[0], 9)).astype(np.float32)
+          old[::5] = 0.0                               # cells without history are not blended (R12)
           ref, rflags = orc.closure_mlp(mom, mlp, tau, min_count=cfg["min_count_mlp"], relax_w=relax_w, coef_old=old)
           coef, flags = ctx.closure_mlp(torch.from_numpy(mom).cuda(), dm, torch.from_numpy(tau).cuda(), relax_w,
                                         coef=torch.from_numpy(old.copy()).cuda())

@@ -104,6 +104,13 @@ def test_features_and_flags(orc):
     old = np.full((4, 9), 7.0)
     c2, _ = orc.closure_mlp(recs, mlp, 2.0, relax_w=0.2, coef_old=old)
     np.testing.assert_allclose(c2[0], 0.2 * coef[0] + 0.8 * 7.0, rtol=1e-14)
+    # ... unless the cell has no history (R12: all nine old coefficients zero, e.g. EMPTY at the previous step)
+    old[0] = 0.0
+    old[2] = 0.0
+    old[3, 4] = 0.0                                            # one zero among nine is still a history
+    c3, _ = orc.closure_mlp(recs, mlp, 2.0, relax_w=0.2, coef_old=old)
+    assert np.array_equal(c3[0], coef[0]) and np.array_equal(c3[2], coef[2])
+    np.testing.assert_allclose(c3[3], 0.2 * coef[3] + 0.8 * old[3], rtol=1e-14)
 
 
 # ------------------------------------------------------------------------------------------------ S6
