@@ -21,11 +21,13 @@
  * stationarity, the drift N_i recovered from the OUTPUT velocities against Eq. 14 typed out in numpy and against
  * the relaxation identities the exact closure imposes (<N_i c_j + N_j c_i> = 0, <N_i c^2 + 2 c_i c.N> = 5 h_i/(3 tau)),
  * an N = 2 cell is updated; walls -- half-range Maxwellian moments on the lid (y-wall) and on both Couette plates
- * (x-walls, distinct tangential wall speeds); diagnostics -- hand values on octahedral ensembles, numpy
+ * (x-walls, distinct tangential wall speeds), the freestream reservoir against the analytic moments of the flux-weighted
+ * drifting half-range Maxwellian at two speed ratios; diagnostics -- hand values on octahedral ensembles, numpy
  * slogdet, rotation invariance, Maxwellian limits, N = 3 cells whose determinant rounds positive.
  * Parity unpinned (no independent source exists): the value of eps^2 (R2-e), the low-count /
- * singular-cell policy (R3-c), the 16-feature definitions (R4), and the wall re-emission details (R7) as
- * compared with the paper's own runs.
+ * singular-cell policy (R3-c), the 16-feature definitions (R4), the wall re-emission details (R7), the reservoir's
+ * algorithm (R11: the law it samples is pinned, that the paper's code does the same is not) and the no-history rule of
+ * the under-relaxation (R12), each as compared with the paper's own runs.
  */
 #include <math.h>
 #include <stdint.h>
