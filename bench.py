@@ -752,7 +752,8 @@ def main():
             extras["paper_surrogate_16_256x4_9"] = paper_surrogate(fpcl, torch, workloads, cfg["tau"])
             extras["c1_couette"] = couette_small(fpcl, torch, workloads)
             extras["c2_closure_microbench"] = closure_microbench(fpcl, torch, workloads, mlp_dev, hbm_peak)
-            extras["c4_ppc_sweep"] = ppc_sweep(fpcl, torch, workloads, 1000 if args.steps >= 100 else 100, steps_20ppc=1000)
+            # BASELINE config 4 asks for the drift after 1,000 steps at every ppc: 0.07 / 0.12 / 0.35 s of GPU time
+            extras["c4_ppc_sweep"] = ppc_sweep(fpcl, torch, workloads, 1000, steps_20ppc=1000)
 
     cpu_baseline = None
     if rank == 0 and not args.no_cpu_baseline:
