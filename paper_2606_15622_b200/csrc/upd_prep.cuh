@@ -14,6 +14,15 @@
 #include "common.cuh"
 
 #define UPD_NC 28                  // floats of per-cell constants
+#ifndef UPD_FAR_S
+#define UPD_FAR_S 1.5                 // drift terms the fast path accepts, in thermal speeds (see [26] below)
+#endif
+#ifndef UPD_FAR_LIN
+#define UPD_FAR_LIN 1.0
+#endif
+#ifndef UPD_FAR_FLOOR
+#define UPD_FAR_FLOOR 4.0            // ... but never a range below (2 sigma)^2
+#endif
 
 // rec: the cell's record (13 or 29 doubles, any address space), cf: its nine coefficients as stored in fp32.
 // Returns FP_FLAG_SKIPPED when the cell holds particles that the update leaves untouched, else 0.
@@ -46,14 +55,36 @@ __device__ __forceinline__ uint32_t upd_prep_cell(const double* rec, int stride,
     o4[3] = make_float4(cf[6], cf[7], cf[8], (float)(eps2 * h0));
     o4[4] = make_float4((float)(eps2 * h1), (float)(eps2 * h2), (float)eps2, (float)(3.0 * theta));
     o4[5] = make_float4((float)E1, (float)((1.0 - E1) * tau), (float)sqrt(theta * (1.0 - E2)), 1.0f);
-    // [26]: in fp32 a drift term T costs ~6e-8 |T| of absolute error; the quadratic and cubic terms of a particle far out in
-    // the cell's distribution, (1-E1) tau |gamma| c^2 and (1-E1) tau eps2 |c|^3, stay below 3 sqrt(theta) (error < 2e-7
-    // sqrt(theta)) as long as |c|^2 < min(3 s / (kap |gamma|), (3 s / (kap eps2))^(2/3)); never below (5 sigma)^2 = 25 theta,
-    // up to where the terms are a few thermal speeds in any physical state.  Equilibrium cells (eps2, gamma ~ 0): infinity.
-    const double kap = (1.0 - E1) * tau, s3 = 3.0 * sqrt(theta);
+    // [26]: in fp32 a drift term T costs ~6e-8 |T| of absolute error per rounding, and the terms of N cancel against each
+    // other.  A particle stays on the fast path while its linear, quadratic and cubic terms, (1-E1) tau |B| |c|,
+    // (1-E1) tau |gamma| c^2 and (1-E1) tau eps2 |c|^3, each stay below UPD_FAR_S thermal speeds, i.e. while
+    // |c|^2 < min((s / (kap |B|))^2, s / (kap |gamma|), (s / (kap eps2))^(2/3)) with s = UPD_FAR_S sqrt(theta); the range is
+    // never taken below UPD_FAR_FLOOR theta.  Equilibrium cells (B, gamma, eps2 ~ 0): infinity.  (Randomised comparison
+    // with the oracle: at 3 thermal speeds and a floor of 25 theta, cells of a few particles -- whose eps2 is
+    // O(1 / (tau theta)) -- missed the 1e-6 tolerance by up to 2x.)
+    const double kap = (1.0 - E1) * tau, s3 = UPD_FAR_S * sqrt(theta);
     const double gmax = fmax(fabs((double)cf[6]), fmax(fabs((double)cf[7]), fabs((double)cf[8])));
     double far2 = fmin(gmax > 0.0 ? s3 / (kap * gmax) : INFINITY, eps2 > 0.0 ? cbrt((s3 / (kap * eps2)) * (s3 / (kap * eps2))) : INFINITY);
-    far2 = fmin(fmax(far2, 25.0 * theta), 3.0e38);
+    {   // the linear term (1-E1) tau |B c| <= kap |B|_inf |c| as well (B = C + I/tau vanishes in equilibrium)
+        const double b0 = fabs((double)cf[0] + itau) + fabs((double)cf[1]) + fabs((double)cf[2]);
+        const double b1 = fabs((double)cf[1]) + fabs((double)cf[3] + itau) + fabs((double)cf[4]);
+        const double b2 = fabs((double)cf[2]) + fabs((double)cf[4]) + fabs((double)cf[5] + itau);
+        const double bmax = fmax(b0, fmax(b1, b2));
+        if (bmax > 0.0) far2 = fmin(far2, (UPD_FAR_LIN * s3 / (kap * bmax)) * (UPD_FAR_LIN * s3 / (kap * bmax)));
+        far2 = fmin(fmax(far2, UPD_FAR_FLOOR * theta), 3.0e38);
+        // The fast path subtracts U as ONE fp32 number: every c of the cell is off by up to d = 2^-24 |U|.  The drift's
+        // Jacobian |dN/dc| <= |B| + 2 |gamma| |c| + 3 eps2 c^2 multiplies that shift: a particle stays on the fast path while
+        // (1-E1) tau |dN/dc| d < 2e-7 thermal speeds.  Binding in hypersonic cells with a strongly non-linear drift (two- and
+        // three-particle cells, whose eps2 is O(1 / (tau theta))): there the bound is below every |c| and the cell always
+        // takes the fp64 path.
+        const double du = 5.97e-8 * fmax(fabs(U0), fmax(fabs(U1), fabs(U2)));
+        const double T = 2.0e-7 * sqrt(theta), A0 = kap * bmax * du, A1 = 2.0 * kap * gmax * du, A2 = 3.0 * kap * eps2 * du;
+        double xu = INFINITY;                                // the |c| at which A2 x^2 + A1 x + A0 reaches T
+        if (A0 >= T) xu = 0.0;
+        else if (A2 > 0.0) xu = (-A1 + sqrt(A1 * A1 + 4.0 * A2 * (T - A0))) / (2.0 * A2);
+        else if (A1 > 0.0) xu = (T - A0) / A1;
+        far2 = fmin(far2, xu * xu);
+    }
     o4[6] = make_float4((float)(tau * tau * (1.0 - E1) * (1.0 - E1) * i3t), (float)(2.0 * tau * (E1 - E2) * i3t), (float)far2, 0.0f);
     return 0u;
 }
