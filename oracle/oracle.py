@@ -142,8 +142,7 @@ def average_results(x, k, avg):
 # ---------------------------------------------------------------- S2/S3
 def _tau_args(tau, ncell):
     if np.ndim(tau) == 0:
-        # the C ABI carries the scalar relaxation time as fp32 (fp_params.tau): hand the oracle the value the library sees
-        return None, C.POINTER(C.c_float)(), float(np.float32(tau))
+        return None, C.POINTER(C.c_float)(), float(tau)
     t = _f32(tau)
     assert t.shape[0] == ncell
     return t, _p(t, C.c_float), 0.0
