@@ -78,7 +78,7 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
               cudaMalloc((void**)&c->bin_total, 512 * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->cellc, (size_t)c->ncell * 28 * 4) == cudaSuccess &&
               cudaMalloc((void**)&c->mom_acc, (size_t)c->ncell * 28 * sizeof(double)) == cudaSuccess &&
-              cudaMalloc((void**)&c->upd_acc, (size_t)c->ncell * 6 * sizeof(double)) == cudaSuccess &&
+              cudaMalloc((void**)&c->upd_acc, (size_t)c->ncell * UPD_ACC * sizeof(double)) == cudaSuccess &&
               cudaHostAlloc((void**)&c->h_err, sizeof(uint32_t), cudaHostAllocMapped) == cudaSuccess &&
               cudaHostGetDevicePointer((void**)&c->d_err, c->h_err, 0) == cudaSuccess &&
               cudaMalloc((void**)&c->d_errdev, 4) == cudaSuccess && cudaMemset(c->d_errdev, 0, 4) == cudaSuccess;

@@ -43,6 +43,8 @@ struct fp_mlp_dev {                 // uploaded copy of the caller's MLP (fp_clo
     bool     valid = false;
 };
 
+#define UPD_ACC 8                  // doubles per cell in upd_acc: seven sums (update.cu: upd_scales), one pad
+
 struct fp_ctx {
     fp_params p;
     int32_t   ncell = 0;
@@ -61,7 +63,7 @@ struct fp_ctx {
     size_t    block_hist_elems = 0;
     float    *cellc = nullptr;       // [ncell * 28] per-cell constants of the velocity update (update.cu)
     double   *mom_acc = nullptr;     // [ncell * 28] raw-sum accumulators of the high-ppc gather (moments_seg.cuh)
-    double   *upd_acc = nullptr;     // [ncell * 6] per-cell sums of the high-ppc update (update_seg.cuh)
+    double   *upd_acc = nullptr;     // [ncell * UPD_ACC] per-cell sums of the high-ppc update (update_seg.cuh)
     // sticky device-side state check (cell_start not a monotone prefix ending at np): one word of mapped pinned host
     // memory that kernels OR into and every entry point reads without synchronising
     uint32_t *h_err = nullptr, *d_err = nullptr;

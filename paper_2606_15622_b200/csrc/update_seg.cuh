@@ -1,19 +1,23 @@
 // update_seg.cuh -- a6 at very high particles per cell (PAPER.md:282 30,000 particles per cell,
 // :491-497 500-1500).  Included by update.cu only.
 //
-// Same arithmetic as upd_giant_cell (pass A per 512-particle slice with all 32 lanes, per-slice sums combined in fp64,
-// fp64 epilogue, pass B as a streaming read-modify-write), but spread over the device: the particle index space is
+// Same arithmetic as upd_giant_cell (pass A in the split form per 512-particle slice with all 32 lanes, per-slice sums
+// combined in fp64, fp64 epilogue upd_scales, pass B as a streaming read-modify-write), but spread over the device: the particle index space is
 // cut into 512-particle slices regardless of cell boundaries, as in moments_seg.cuh.
 //   upd_seg_a_kernel: a warp stages its slice (vx, vy, vz, pid: four aligned bulk copies), runs pass A for every cell
-//     that intersects it (un-normalised c* over the velocities, six partial sums), adds the sums to the cell's fp64
+//     that intersects it (w = E1 v + q' over the velocities, seven partial sums), adds the sums to the cell's fp64
 //     accumulators with atomics and writes the slice back with bulk stores;
 //   upd_seg_b_kernel: a warp walks the cells of its slice again, forms alpha / the recentring mean / the energy scale
 //     from the accumulators exactly as upd_giant_cell does, and rewrites its part of the cell.
+// No cell is handed to the fp64 path here (the velocities are overwritten slice by slice before a cell's range is known):
+// a particle beyond its cell's fp32 range (upd_prep.cuh [26]) keeps the fast path's accuracy, about 1e-6 of the drift term.
 // 52 instead of 28 B per particle, every SM busy: 300 cells x 30,000 particles 1.55 ms -> see DESIGN.md.
 #pragma once
 
 #define UPD_SEG 512
 #define UPD_SEG_WARPS 4
+#define UPD_SEG_TINY 8                 // cells of at most this many particles take the fp64 path (conservation scales of a
+                                   // few-particle cell amplify fp32 rounding, see upd_finish)
 
 __device__ __forceinline__ int32_t upd_seg_first_cell(const int32_t* __restrict__ cell_start, int32_t ncell, int32_t a)
 {
@@ -64,6 +68,7 @@ upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restri
             if (cs0 >= b) break;
             const int32_t s = max(cs0, a), e = min(cs1, b);
             if (e <= s) continue;
+            if (cs1 - cs0 <= UPD_SEG_TINY) continue;             // left untouched for the fp64 path in upd_seg_b_kernel
             float k[UPD_NC];
             const float* cc = cellc + (size_t)c * UPD_NC;
 #pragma unroll
@@ -72,22 +77,23 @@ upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restri
                 k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
             }
             if (k[23] == 0.0f) continue;                         // inactive cell: velocities stay
-            const upd_part pa = upd_pass_a<32>(sx, sy, sz, sp, s - a, e - s, lane, k, Q);
-            double D[6] = {(double)(pa.SNN.x + pa.SNN.y), (double)(pa.SCN.x + pa.SCN.y), (double)(pa.SM0.x + pa.SM0.y),
-                           (double)(pa.SM1.x + pa.SM1.y), (double)(pa.SM2.x + pa.SM2.y), (double)(pa.SQ.x + pa.SQ.y)};
+            const upd_part pa = upd_pass_a<32, true>(sx, sy, sz, sp, s - a, e - s, lane, k, Q);
+            double D[7] = {(double)(pa.SNN.x + pa.SNN.y), (double)(pa.SCN.x + pa.SCN.y), (double)(pa.SM0.x + pa.SM0.y),
+                           (double)(pa.SM1.x + pa.SM1.y), (double)(pa.SM2.x + pa.SM2.y), (double)(pa.SQ.x + pa.SQ.y),
+                           (double)(pa.SCQ.x + pa.SCQ.y)};
 #pragma unroll
             for (int d = 16; d >= 1; d >>= 1) {
 #pragma unroll
-                for (int q = 0; q < 6; ++q) D[q] += fpd_shfl_xor(D[q], d);
+                for (int q = 0; q < 7; ++q) D[q] += fpd_shfl_xor(D[q], d);
             }
-            if (lane < 6) {
+            if (lane < 7) {
                 double mine = D[0];
 #pragma unroll
-                for (int q = 1; q < 6; ++q) if (lane == q) mine = D[q];
-                atomicAdd(&acc[(size_t)c * 6 + lane], mine);
+                for (int q = 1; q < 7; ++q) if (lane == q) mine = D[q];
+                atomicAdd(&acc[(size_t)c * UPD_ACC + lane], mine);
             }
         }
-        // ---- c* back to global memory: aligned part by bulk stores, the ragged end of the last slice by plain stores
+        // ---- w = E1 v + q' back to global memory: aligned part by bulk stores, the ragged end of the last slice by plain stores
         fpt_fence_proxy_async();
         __syncwarp();
         if (lane == 0 && nb > 0) {
@@ -119,6 +125,7 @@ upd_seg_b_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restri
             if (cs0 >= b) break;
             const int32_t s = max(cs0, a), e = min(cs1, b);
             if (e <= s) continue;
+            if (cs1 - cs0 <= UPD_SEG_TINY) continue;             // upd_seg_tiny_kernel
             float k[UPD_NC];
             const float* cc = cellc + (size_t)c * UPD_NC;
 #pragma unroll
@@ -127,24 +134,36 @@ upd_seg_b_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restri
                 k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
             }
             if (k[23] == 0.0f) continue;
-            const double* D = acc + (size_t)c * 6;
-            const double invn = 1.0 / (double)(cs1 - cs0);
-            const double alpha2 = 1.0 + ((double)k[24] * D[0] + (double)k[25] * D[1]) * invn;
-            double alpha = 1.0;
-            if (!isfinite(alpha2) || alpha2 < 1e-6) { if (lane == 0 && cs0 >= a) flags[c] |= FP_FLAG_ALPHA; }   // once per cell
-            else alpha = sqrt(alpha2);
-            float mm0 = 0.f, mm1 = 0.f, mm2 = 0.f, scale = (float)(1.0 / alpha);
-            if (Q.conserve_mode == 1) {
-                const double m0 = D[2] * invn, m1 = D[3] * invn, m2 = D[4] * invn;
-                const double en = D[5] * invn - (m0 * m0 + m1 * m1 + m2 * m2);
-                mm0 = (float)m0; mm1 = (float)m1; mm2 = (float)m2;
-                if (en > 0.0 && isfinite(en)) scale = (float)sqrt((double)k[19] / en);
-            }
+            float sc, f0, f1, f2;
+            if (!upd_scales(k, acc + (size_t)c * UPD_ACC, cs1 - cs0, Q.conserve_mode, sc, f0, f1, f2) && lane == 0 && cs0 >= a)
+                flags[c] |= FP_FLAG_ALPHA;                        // once per cell
             for (int32_t p = s + lane; p < e; p += 32) {
-                vx[p] = k[0] + fmaf(vx[p] - mm0, scale, k[3]);
-                vy[p] = k[1] + fmaf(vy[p] - mm1, scale, k[4]);
-                vz[p] = k[2] + fmaf(vz[p] - mm2, scale, k[5]);
+                vx[p] = fmaf(vx[p], sc, f0);
+                vy[p] = fmaf(vy[p], sc, f1);
+                vz[p] = fmaf(vz[p], sc, f2);
             }
         }
+    }
+}
+
+// The cells of at most UPD_SEG_TINY particles, which the two kernels above leave untouched: one warp per 32 cells, each such
+// cell redone by the whole warp on the fp64 path (its own kernel: the call would cost upd_seg_b_kernel 88 registers).
+__global__ void __launch_bounds__(128)
+upd_seg_tiny_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
+                    const int32_t* __restrict__ cell_start, uint32_t* __restrict__ flags, const uint32_t* __restrict__ err_dev,
+                    const __grid_constant__ upd_src R, const __grid_constant__ upd_params Q)
+{
+    fpd_pdl();
+    if (*err_dev) return;
+    const int lane = threadIdx.x & 31;
+    const int32_t c0 = (int32_t)((blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32);
+    if (c0 >= Q.ncell) return;
+    const int32_t c = c0 + lane;
+    const int32_t n = c < Q.ncell ? cell_start[c + 1] - cell_start[c] : 0;
+    uint32_t tiny = __ballot_sync(0xffffffffu, n >= 2 && n <= UPD_SEG_TINY);
+    while (tiny) {
+        const int j = __ffs(tiny) - 1;
+        tiny &= tiny - 1;
+        upd_far_cell(vx, vy, vz, pid, cell_start, R, flags, c0 + j, Q);
     }
 }
