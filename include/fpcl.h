@@ -256,14 +256,15 @@ int fp_step(fp_ctx* ctx, int64_t np,
  * fp_collide: the part of fp_step after the move -- sort by cell, moments, closure, update -- with fp_step's arguments;
  * positions are read only. */
 int fp_set_slab(fp_ctx* ctx, int32_t row0, int32_t nrows);
-/* on != 0: every per-cell result depends only on the cell's own particles in their array order, not on WHERE in the arrays
- * they sit.  By default the moment gather starts each cell at the particle whose shared-memory bank suits the warp (no bank
- * conflicts, ~4 us at 4M particles), which makes the fp32 summation order -- not the result beyond rounding -- depend on the
- * cell's offset.  Switch it on (on every slab and on the uncut run) to compare decompositions bit for bit.  What stays
- * context-dependent: the lanes-per-cell width G is chosen from the context's mean particles per cell (thresholds 56/112/224),
- * and a warp's chunk of 32/G cells, counted from the slab's first cell, that overflows the 512-particle staging buffer is
- * walked by the whole warp in another order.  Slabs whose mean density falls on the other side of a threshold, or whose
- * chunks overflow where the uncut run's do not, agree with the uncut run to rounding only. */
+/* on != 0: every per-cell result (moment record, coefficients, updated velocities) depends only on the cell's own particles
+ * in their array order -- not on WHERE in the arrays they sit, on the cell's neighbours, on the context's mean density, nor on
+ * the run.  By default the moment gather and the velocity update give a group of 4..32 lanes one cell and pick the group
+ * width from the context's mean particles per cell, start each cell at the particle whose shared-memory bank suits the
+ * warp, and send ensembles of few huge cells through slice kernels that combine per-slice sums with atomics: all of
+ * that changes the fp32 summation ORDER -- not the result beyond rounding -- with the cell's offset and surroundings.
+ * Reproducible mode walks every cell on its own with all 32 lanes and never uses the slice kernels (2-3x slower moments
+ * and update at 100 particles per cell).  Switch it on (on every slab and on the uncut run) to compare decompositions bit
+ * for bit. */
 int fp_set_reproducible(fp_ctx* ctx, int32_t on);
 int fp_slab_partition(fp_ctx* ctx, int64_t np,
                       const float* x, const float* y, const float* vx, const float* vy, const float* vz, const uint32_t* pid,

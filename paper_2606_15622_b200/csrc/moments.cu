@@ -484,7 +484,12 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
         return fpd_cells_ok(v, c * CPW, cells, ncell, np, lane, err) ? v : 0;
     };
     auto range_of = [&](int32_t cs) {
-        return fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, (aligned & 1) != 0, MOM_CAP);
+        fpw_range r = fpw_range_of(__shfl_sync(0xffffffffu, cs, 0), __shfl_sync(0xffffffffu, cs, CPW), np, (aligned & 1) != 0, MOM_CAP);
+        // fp_set_reproducible: every cell on its own with all 32 lanes (mom_dense_chunk), so that a cell's summation order
+        // depends on nothing but the cell -- not on its neighbours in the chunk, nor on the lanes-per-cell width the
+        // context's mean density selects
+        if (aligned & 2) r.staged = false;
+        return r;
     };
     auto issue = [&](const fpw_range& r, int b) {
         const uint32_t bytes = (uint32_t)r.nb * 4u;
@@ -614,7 +619,8 @@ extern "C" int fp_cell_moments(fp_ctx* ctx, int64_t np, const float* vx, const f
     // (with at least one resident warp's worth of cells per warp slot, one warp per huge cell is still the faster
     // path: 4096 cells x 1000 particles 39 vs 46 us; 300 cells x 30,000 particles 367 vs 60 us)
     const bool few_cells = ctx->ncell < ctx->num_sms * 16 || ctx->env_mom_seg;
-    if (ppc > MOM_SEG_MIN && few_cells && aligned16 && np > 0 && np < ((int64_t)1 << 31) && !ctx->env_mom_no_seg) {
+    // (not in reproducible mode: the slices add to a cell's accumulators with atomics, in an order that varies from run to run)
+    if (ppc > MOM_SEG_MIN && few_cells && aligned16 && np > 0 && np < ((int64_t)1 << 31) && !ctx->env_mom_no_seg && !ctx->reproducible) {
         const size_t bytes = (size_t)ctx->ncell * 28 * sizeof(double);       // allocated at fp_create
         fp_launch(fp_cs_check_kernel, fp_div_up(ctx->ncell + 1, 256) < 296 ? fp_div_up(ctx->ncell + 1, 256) : 296, 256, 0, st, cell_start,
                   ctx->ncell, np, ctx->d_err, ctx->d_errdev);
