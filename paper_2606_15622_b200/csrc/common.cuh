@@ -43,6 +43,7 @@ struct fp_mlp_dev {                 // uploaded copy of the caller's MLP (fp_clo
     bool     valid = false;
 };
 
+#define SW_TB_CAP 4095               // entries of the reservoir's tie-break list (expected: a handful per step at 20M particles)
 #define UPD_ACC 8                  // doubles per cell in upd_acc: seven sums (update.cu: upd_scales), one pad
 
 struct fp_ctx {
@@ -68,6 +69,7 @@ struct fp_ctx {
     // memory that kernels OR into and every entry point reads without synchronising
     uint32_t *h_err = nullptr, *d_err = nullptr;
     uint32_t *d_errdev = nullptr;    // device-memory copy of the word for kernels that must not run on bad boundaries
+    uint32_t *d_tiebreak = nullptr;  // [1 + SW_TB_CAP]: count + particle indices whose reservoir accept/reject test was borderline in fp32
     int       mom_occ[6] = {0, 0, 0, 0, 0, 0};       // resident CTAs per SM of moments_warp_kernel<2^k, *>
     int       mlp_tc_occ = 0, sw_occ[2] = {0, 0}, gather_occ = 0;
     bool      mlp_attr_w5 = false, mlp_attr_wd = false;

@@ -17,6 +17,7 @@ struct sw_params {
     uint32_t k0, k1, step_lo, step_hi;
     fp_grid grid;                    // cell keys (slab-aware)
     float in_mu, in_sg, in_pen;     // freestream reservoir: mode of the flux density, sqrt(theta_inf), fl(U_inf,x * dt)
+    uint32_t* tiebreak;              // [0] count, [1..] indices of re-inserted particles with a borderline fp32 accept/reject test
 };
 
 // One wall draw (R7): normal component sqrt(-2 theta_w ln u0) into the gas, tangentials
@@ -38,28 +39,34 @@ __device__ __forceinline__ void sw_wall_draw(const sw_params& P, uint32_t pid, u
 // v > 0, by acceptance-rejection about the mode mu (candidate mu + sigma z, accepted iff v > 0 and (v/mu) e^(1 - v/mu) >= u2;
 // attempt a uses the Philox stream 16 + a, a < 8; then v = mu); tangentials and the entry position from stream 32.  The
 // position follows a fixed fp32 sequence (it decides the cell index).  The accept / reject test DECIDES which attempt's
-// candidate the particle gets, so it is evaluated in fp64 like the oracle's (an fp32 test flips once in ~1e6 draws: found
-// by randomised comparison on 1.2M particles); this path runs for the few particles that leave through an open face.
-__device__ __forceinline__ double sw_uniform_f64(uint32_t w) { return ((double)(w >> 9) + 0.5) * (1.0 / 8388608.0); }
-
-__device__ __noinline__ void sw_reinsert(const sw_params& P, uint32_t pid, bool two_d, float& xp, float& yp, float& v0,
+// candidate the particle gets.  It is evaluated in fp32 here; a particle with a test within 1e-4 of the line (a hundred
+// times the fp32 error) is put on a list and sw_tiebreak_kernel repeats its whole draw in fp64, the oracle's precision.
+// (An unguarded fp32 test flipped once in ~1e6 draws, found by randomised comparison on 1.2M particles; fp64 arithmetic
+// anywhere in this kernel's call tree costs it its 64 registers: 177 -> 300 us at 20M particles.)
+__device__ __noinline__ void sw_reinsert(const sw_params& P, uint32_t pid, uint32_t p, bool two_d, float& xp, float& yp, float& v0,
                                          float& v1, float& v2)
 {
-    const double th = (double)P.wall[0].theta_w, U = (double)P.wall[0].ux, sg = sqrt(th), mu = 0.5 * (U + sqrt(U * U + 4.0 * th));
-    double vn = mu;
+    float vn = P.in_mu;
+    bool borderline = false;
     for (uint32_t a = 0; a < 8u; ++a) {
         const uint4 w = fpd_philox4x32_10(pid, P.step_lo, P.step_hi, 16u + a, P.k0, P.k1);
-        double s, c;
-        sincospi(2.0 * sw_uniform_f64(w.y), &s, &c);
-        const double cand = mu + sg * sqrt(-2.0 * log(sw_uniform_f64(w.x))) * c;
-        const double q = cand / mu;
-        if (cand > 0.0 && q * exp(1.0 - q) >= sw_uniform_f64(w.z)) { vn = cand; break; }
+        float s, c;
+        sincospif(2.0f * fpd_uniform(w.y), &s, &c);
+        const float cand = fmaf(P.in_sg * sqrtf(-2.0f * logf(fpd_uniform(w.x))), c, P.in_mu);
+        const float q = cand / P.in_mu;
+        const float lhs = q * expf(1.0f - q), rhs = fpd_uniform(w.z);
+        borderline = borderline || fabsf(lhs - rhs) < 1.0e-4f || fabsf(cand) < 1.0e-4f * P.in_sg;
+        if (cand > 0.0f && lhs >= rhs) { vn = cand; break; }
+    }
+    if (borderline) {
+        const uint32_t slot = atomicAdd(P.tiebreak, 1u);
+        if (slot < SW_TB_CAP) P.tiebreak[1 + slot] = p;
     }
     const uint4 w = fpd_philox4x32_10(pid, P.step_lo, P.step_hi, 32u, P.k0, P.k1);
     const float r = P.in_sg * sqrtf(-2.0f * logf(fpd_uniform(w.x)));
     float s, c;
     sincospif(2.0f * fpd_uniform(w.y), &s, &c);
-    v0 = (float)vn; v1 = fmaf(r, c, P.wall[0].uy); v2 = fmaf(r, s, P.wall[0].uz);
+    v0 = vn; v1 = fmaf(r, c, P.wall[0].uy); v2 = fmaf(r, s, P.wall[0].uz);
     float xn = __fadd_rn(P.xmin, __fmul_rn(fpd_uniform(w.w), P.in_pen));
     if (xn < P.xmin) xn = P.xmin;
     if (xn >= P.xmax) xn = P.xmax_in;
@@ -101,7 +108,7 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
                     if (xp < P.xmin) xp = P.xmin;
                     if (xp >= P.xmax) xp = P.xmax_in;
                 } else if (INFLOW && w.kind == FP_WALL_INFLOW) {
-                    sw_reinsert(P, pid[p], P.ny > 1, xp, yp, v0, v1, v2);
+                    sw_reinsert(P, pid[p], (uint32_t)p, P.ny > 1, xp, yp, v0, v1, v2);
                     redrawn = true; reinserted = true;
                 }
             }
@@ -124,7 +131,7 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
                     if (yp < P.ymin) yp = P.ymin;
                     if (yp >= P.ymax) yp = P.ymax_in;
                 } else if (INFLOW && w.kind == FP_WALL_INFLOW) {
-                    sw_reinsert(P, pid[p], true, xp, yp, v0, v1, v2);
+                    sw_reinsert(P, pid[p], (uint32_t)p, true, xp, yp, v0, v1, v2);
                     redrawn = true;
                 }
             }
@@ -168,8 +175,10 @@ __device__ __forceinline__ void sw_hist(uint32_t* __restrict__ tile_hist, int nt
 // One particle per thread, grid-stride.  (Four particles per thread with 128-bit accesses was measured slower:
 // 37 vs 33 us at 4M particles.)
 // INFLOW: the grid has freestream faces (the re-insertion's call and registers stay out of the other instantiation).
+// (the reservoir variant is held to 64 registers -- four resident blocks: this kernel lives on loads in flight, 177 us at
+// 20M particles against 217 us with the 80 registers the re-insertion's call would otherwise take; the others to 40: six blocks)
 template <bool WRITE_KEYS, bool INFLOW>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, INFLOW ? 4 : 6)
 sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
           float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
           uint32_t* __restrict__ keys, uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask,
@@ -191,6 +200,32 @@ sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __res
         }
         if (WRITE_KEYS && tile_hist) sw_hist(tile_hist, ntiles, p0 / SORT_TILE, valid, key, digit_mask, lane);
     }
+}
+
+// The listed particles' normal velocity again, every attempt's test in fp64 (as the oracle evaluates it); resets the list.
+__device__ __forceinline__ double sw_uniform_f64(uint32_t w) { return ((double)(w >> 9) + 0.5) * (1.0 / 8388608.0); }
+
+__global__ void __launch_bounds__(128)
+sw_tiebreak_kernel(float* __restrict__ vx, const uint32_t* __restrict__ pid, const __grid_constant__ sw_params P)
+{
+    fpd_pdl();
+    const uint32_t n = min(P.tiebreak[0], (uint32_t)SW_TB_CAP);
+    const double th = (double)P.wall[0].theta_w, U = (double)P.wall[0].ux, sg = sqrt(th), mu = 0.5 * (U + sqrt(U * U + 4.0 * th));
+    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+        const uint32_t p = P.tiebreak[1 + i];
+        double vn = mu;
+        for (uint32_t a = 0; a < 8u; ++a) {
+            const uint4 w = fpd_philox4x32_10(pid[p], P.step_lo, P.step_hi, 16u + a, P.k0, P.k1);
+            double s, c;
+            sincospi(2.0 * sw_uniform_f64(w.y), &s, &c);
+            const double cand = mu + sg * sqrt(-2.0 * log(sw_uniform_f64(w.x))) * c;
+            const double q = cand / mu;
+            if (cand > 0.0 && q * exp(1.0 - q) >= sw_uniform_f64(w.z)) { vn = cand; break; }
+        }
+        vx[p] = (float)vn;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) P.tiebreak[0] = 0u;
 }
 
 int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
@@ -217,6 +252,7 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
         P.in_sg = (float)sqrt(th);
         volatile float pen = q.wall[0].ux * q.dt; P.in_pen = pen;
     }
+    P.tiebreak = ctx->d_tiebreak;
     P.k0 = (uint32_t)q.seed; P.k1 = (uint32_t)(q.seed >> 32);
     P.step_lo = (uint32_t)step; P.step_hi = (uint32_t)(step >> 32);
     const int threads = 256;
@@ -244,8 +280,9 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
         if (inflow) fp_launch(sw_kernel<false, true>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
         else        fp_launch(sw_kernel<false, false>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
     }
+    if (inflow) fp_launch(sw_tiebreak_kernel, 1, 128, 0, st, vx, pid, P);
     FP_LAUNCH_OK(ctx);
-    FP_COUNT(ctx, 1);
+    FP_COUNT(ctx, inflow ? 2 : 1);
     return FP_OK;
 }
 
