@@ -17,9 +17,6 @@
 #ifndef UPD_FAR_S
 #define UPD_FAR_S 1.5                 // drift terms the fast path accepts, in thermal speeds (see [26] below)
 #endif
-#ifndef UPD_FAR_LIN
-#define UPD_FAR_LIN 1.0
-#endif
 #ifndef UPD_FAR_FLOOR
 #define UPD_FAR_FLOOR 4.0            // ... but never a range below (2 sigma)^2
 #endif
@@ -70,7 +67,7 @@ __device__ __forceinline__ uint32_t upd_prep_cell(const double* rec, int stride,
         const double b1 = fabs((double)cf[1]) + fabs((double)cf[3] + itau) + fabs((double)cf[4]);
         const double b2 = fabs((double)cf[2]) + fabs((double)cf[4]) + fabs((double)cf[5] + itau);
         const double bmax = fmax(b0, fmax(b1, b2));
-        if (bmax > 0.0) far2 = fmin(far2, (UPD_FAR_LIN * s3 / (kap * bmax)) * (UPD_FAR_LIN * s3 / (kap * bmax)));
+        if (bmax > 0.0) far2 = fmin(far2, (s3 / (kap * bmax)) * (s3 / (kap * bmax)));
         far2 = fmin(fmax(far2, UPD_FAR_FLOOR * theta), 3.0e38);
         // The fast path subtracts U as ONE fp32 number: every c of the cell is off by up to d = 2^-24 |U|.  The drift's
         // Jacobian |dN/dc| <= |B| + 2 |gamma| |c| + 3 eps2 c^2 multiplies that shift: a particle stays on the fast path while
