@@ -9,7 +9,8 @@
 // layout of the constants: [0..2] U_hi, [3..5] U_lo, [6..11] B = C + I/tau (11,12,13,22,23,33), [12..14] gamma,
 // [15..17] eps2*h, [18] eps2, [19] 3 theta, [20] E1, [21] (1-E1) tau, [22] sqrt(theta (1-E2)), [23] active,
 // [24] tau^2 (1-E1)^2 / (3 theta), [25] 2 tau (E1-E2) / (3 theta),
-// [26] |c|^2 beyond which a particle's drift is re-evaluated in fp64 (see upd_far_kernel in update.cu)
+// [26] |c|^2 beyond which a particle's drift is re-evaluated in fp64 (upd_far_cell in update.cu), [27] the same for the paths
+// that give a cell all 32 lanes and subtract U as hi + lo (no bulk-velocity rounding shift)
 #pragma once
 #include "common.cuh"
 
@@ -61,6 +62,7 @@ __device__ __forceinline__ uint32_t upd_prep_cell(const double* rec, int stride,
     // O(1 / (tau theta)) -- missed the 1e-6 tolerance by up to 2x.)
     const double kap = (1.0 - E1) * tau, s3 = UPD_FAR_S * sqrt(theta);
     const double gmax = fmax(fabs((double)cf[6]), fmax(fabs((double)cf[7]), fabs((double)cf[8])));
+    double far2_hl;
     double far2 = fmin(gmax > 0.0 ? s3 / (kap * gmax) : INFINITY, eps2 > 0.0 ? cbrt((s3 / (kap * eps2)) * (s3 / (kap * eps2))) : INFINITY);
     {   // the linear term (1-E1) tau |B c| <= kap |B|_inf |c| as well (B = C + I/tau vanishes in equilibrium)
         const double b0 = fabs((double)cf[0] + itau) + fabs((double)cf[1]) + fabs((double)cf[2]);
@@ -80,8 +82,9 @@ __device__ __forceinline__ uint32_t upd_prep_cell(const double* rec, int stride,
         if (A0 >= T) xu = 0.0;
         else if (A2 > 0.0) xu = (-A1 + sqrt(A1 * A1 + 4.0 * A2 * (T - A0))) / (2.0 * A2);
         else if (A1 > 0.0) xu = (T - A0) / A1;
+        far2_hl = far2;                                      // [27]: the range of the paths that subtract U as hi + lo (32 lanes per cell)
         far2 = fmin(far2, xu * xu);
     }
-    o4[6] = make_float4((float)(tau * tau * (1.0 - E1) * (1.0 - E1) * i3t), (float)(2.0 * tau * (E1 - E2) * i3t), (float)far2, 0.0f);
+    o4[6] = make_float4((float)(tau * tau * (1.0 - E1) * (1.0 - E1) * i3t), (float)(2.0 * tau * (E1 - E2) * i3t), (float)far2, (float)far2_hl);
     return 0u;
 }

@@ -9,8 +9,8 @@
 //     accumulators with atomics and writes the slice back with bulk stores;
 //   upd_seg_b_kernel: a warp walks the cells of its slice again, forms alpha / the recentring mean / the energy scale
 //     from the accumulators exactly as upd_giant_cell does, and rewrites its part of the cell.
-// No cell is handed to the fp64 path here (the velocities are overwritten slice by slice before a cell's range is known):
-// a particle beyond its cell's fp32 range (upd_prep.cuh [26]) keeps the fast path's accuracy, about 1e-6 of the drift term.
+// A particle beyond its cell's fp32 range (upd_prep.cuh [26]) gets its w recomputed in fp64 while its slice is still in
+// shared memory (upd_fix_far_slice); cells of at most UPD_SEG_TINY particles are left to upd_seg_tiny_kernel.
 // 52 instead of 28 B per particle, every SM busy: 300 cells x 30,000 particles 1.55 ms -> see DESIGN.md.
 #pragma once
 
@@ -32,7 +32,8 @@ __device__ __forceinline__ int32_t upd_seg_first_cell(const int32_t* __restrict_
 __global__ void __launch_bounds__(UPD_SEG_WARPS * 32)
 upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
                  const int32_t* __restrict__ cell_start, int64_t np, const float* __restrict__ cellc,
-                 double* __restrict__ acc, const uint32_t* __restrict__ err_dev, const __grid_constant__ upd_params Q)
+                 double* __restrict__ acc, const uint32_t* __restrict__ err_dev, const __grid_constant__ upd_src R,
+                 const __grid_constant__ upd_params Q)
 {
     fpd_pdl();
     if (*err_dev) return;                                   // cell_start failed fp_cs_check_kernel: touch nothing
@@ -78,6 +79,12 @@ upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restri
             }
             if (k[23] == 0.0f) continue;                         // inactive cell: velocities stay
             const upd_part pa = upd_pass_a<32, true>(sx, sy, sz, sp, s - a, e - s, lane, k, Q);
+            if (__any_sync(0xffffffffu, pa.far > k[27])) {       // particles beyond the cell's fp32 range: their w again, in fp64
+                __syncwarp();
+                upd_fix_far_slice(vx + s, vy + s, vz + s, pid + s, sx + (s - a), sy + (s - a), sz + (s - a), e - s, lane, R, c,
+                                  cc, Q);
+                __syncwarp();
+            }
             double D[7] = {(double)(pa.SNN.x + pa.SNN.y), (double)(pa.SCN.x + pa.SCN.y), (double)(pa.SM0.x + pa.SM0.y),
                            (double)(pa.SM1.x + pa.SM1.y), (double)(pa.SM2.x + pa.SM2.y), (double)(pa.SQ.x + pa.SQ.y),
                            (double)(pa.SCQ.x + pa.SCQ.y)};
