@@ -218,7 +218,13 @@ int fp_cell_sixth_moment(fp_ctx* ctx, int64_t np, const float* vx, const float* 
                 const int32_t* cell_start, const double* mom, int32_t mom_stride, double* dm6, void* stream);
 
 /* a6 -- FP velocity update, in place on cell-sorted vx, vy, vz (Eq. 13-15 :150-181; R5, R6).
- * step is the Philox counter word for time.  flags [ncell] are OR-ed with FP_FLAG_ALPHA / FP_FLAG_SKIPPED. */
+ * step is the Philox counter word for time.  flags [ncell] are OR-ed with FP_FLAG_ALPHA / FP_FLAG_SKIPPED.
+ * mom, coef and tau_cell must be the arrays the coefficients were computed from and stay valid until the call has run:
+ * besides the per-cell constants derived from them, the kernel re-reads them for the cells it redoes in fp64 (cells with a
+ * particle beyond the range fp32 arithmetic holds to 1e-6, few-particle cells whose conservation scale cancels; DESIGN.md
+ * section 5).  Accuracy: 1e-6 * max(|v|, sqrt(theta_cell)) per component against Eq. 13-15 evaluated in fp64 with the
+ * same Philox stream.  Grids of few huge cells (above ~450 particles per cell) run slice kernels that add per-slice sums
+ * with fp64 atomics: their results can differ in the last bit from run to run (fp_set_reproducible avoids them). */
 int fp_velocity_update(fp_ctx* ctx, int64_t np, float* vx, float* vy, float* vz, const uint32_t* pid,
                        const int32_t* cell_start, const double* mom, int32_t mom_stride, const float* coef,
                        const float* tau_cell /* nullable */, uint64_t step, uint32_t* flags, void* stream);
