@@ -231,7 +231,7 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
 typedef fp_grid gather_grid;
 
 template <bool FROM_POS>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 6)                   // 40 registers: all eight gathers of a trip in flight
 gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ skeys, int32_t ncell,
               int32_t* __restrict__ cell_start,
               const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ vx,
@@ -245,15 +245,23 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
     const int lane = threadIdx.x & 31;
     const int kfirst = (int)(blockIdx.x * blockDim.x + (threadIdx.x & ~31));
     uint32_t s_pref = (kfirst + lane < n) ? perm[kfirst + lane] : 0u;      // the permutation entry is fetched one trip ahead
+    // lane 0 also needs the key of position k0 - 1 (its left neighbour belongs to another warp): that entry is fetched one
+    // trip ahead too, and its positions are gathered together with the trip's own (as a dependent chain after them --
+    // perm[k0 - 1], then x and y -- it made the whole warp wait twice more per trip: 11 % of the kernel's stall samples)
+    uint32_t l_pref = (FROM_POS && lane == 0 && kfirst > 0 && kfirst < n) ? perm[kfirst - 1] : 0u;
     for (int k0 = kfirst; k0 < n; k0 += stride) {                           // warp-uniform
         const int k = k0 + lane;
         const bool valid = k < n;
         int key = 0, lo = 0;
-        float px = 0.f, py = 0.f;
-        const uint32_t s = s_pref;
+        float px = 0.f, py = 0.f, pvx = 0.f, pvy = 0.f, pvz = 0.f, lx = 0.f, ly = 0.f;
+        uint32_t ppid = 0u;
+        const uint32_t s = s_pref, sl = l_pref;
         if ((int64_t)k + stride < n) s_pref = perm[k + stride];
+        if (FROM_POS && lane == 0 && (int64_t)k0 + stride < n) l_pref = perm[k0 + stride - 1];
         if (valid) {
-            px = x[s]; py = y[s];
+            // every gather of the trip is issued before the first use
+            px = x[s]; py = y[s]; pvx = vx[s]; pvy = vy[s]; pvz = vz[s]; ppid = pid[s];
+            if (FROM_POS && lane == 0 && k > 0) { lx = x[sl]; ly = y[sl]; }
             if (FROM_POS) {
                 key = fpd_cell_key(px, py, Gd);
             } else {
@@ -263,14 +271,11 @@ gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __r
         }
         if (FROM_POS) {
             int prev = __shfl_up_sync(0xffffffffu, key, 1);
-            if (lane == 0 && k > 0 && valid) {
-                const uint32_t s2 = perm[k - 1];
-                prev = fpd_cell_key(x[s2], y[s2], Gd);
-            }
+            if (lane == 0 && k > 0 && valid) prev = fpd_cell_key(lx, ly, Gd);
             lo = (k == 0) ? 0 : prev + 1;
         }
         if (valid) {
-            xo[k] = px; yo[k] = py; vxo[k] = vx[s]; vyo[k] = vy[s]; vzo[k] = vz[s]; pido[k] = pid[s];
+            xo[k] = px; yo[k] = py; vxo[k] = pvx; vyo[k] = pvy; vzo[k] = pvz; pido[k] = ppid;
             for (int c = lo; c <= key; ++c) cell_start[c] = k;
             if (k == n - 1) for (int c = key + 1; c <= ncell; ++c) cell_start[c] = n;
         }
