@@ -19,7 +19,9 @@
 #define UPD_FAR_S 1.5                 // drift terms the fast path accepts, in thermal speeds (see [26] below)
 #endif
 #ifndef UPD_FAR_FLOOR
-#define UPD_FAR_FLOOR 4.0            // ... but never a range below (2 sigma)^2
+#define UPD_FAR_FLOOR 1.0            // ... but never a range below sigma^2 (4.0 left particles at 1.6-2 sigma of bimodal
+                                     // Mach-9 cells, cubic term ~5 thermal speeds, on the fast path: up to 1.85x the tolerance;
+                                     // the step time does not depend on it: those cells hold a particle beyond 2 sigma anyway)
 #endif
 
 // rec: the cell's record (13 or 29 doubles, any address space), cf: its nine coefficients as stored in fp32.

@@ -79,15 +79,15 @@ upd_seg_a_kernel(float* __restrict__ vx, float* __restrict__ vy, float* __restri
             }
             if (k[23] == 0.0f) continue;                         // inactive cell: velocities stay
             const upd_part pa = upd_pass_a<32, true>(sx, sy, sz, sp, s - a, e - s, lane, k, Q);
-            if (__any_sync(0xffffffffu, pa.far > k[27])) {       // particles beyond the cell's fp32 range: their w again, in fp64
-                __syncwarp();
-                upd_fix_far_slice(vx + s, vy + s, vz + s, pid + s, sx + (s - a), sy + (s - a), sz + (s - a), e - s, lane, R, c,
-                                  cc, Q);
-                __syncwarp();
-            }
             double D[7] = {(double)(pa.SNN.x + pa.SNN.y), (double)(pa.SCN.x + pa.SCN.y), (double)(pa.SM0.x + pa.SM0.y),
                            (double)(pa.SM1.x + pa.SM1.y), (double)(pa.SM2.x + pa.SM2.y), (double)(pa.SQ.x + pa.SQ.y),
                            (double)(pa.SCQ.x + pa.SCQ.y)};
+            if (__any_sync(0xffffffffu, pa.far > k[27])) {       // particles beyond the cell's fp32 range: their w and their
+                __syncwarp();                                    // terms of the sums again, in fp64
+                upd_fix_far_slice(vx + s, vy + s, vz + s, pid + s, sx + (s - a), sy + (s - a), sz + (s - a), e - s, lane, R, c,
+                                  cc, Q, D);
+                __syncwarp();
+            }
 #pragma unroll
             for (int d = 16; d >= 1; d >>= 1) {
 #pragma unroll
