@@ -163,6 +163,53 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
     }
 }
 
+// Cross-lane sums of the group's partial records through shared memory: every lane stores its NP partial sums as one row
+// (row stride NP + 4 floats: 128-bit stores, and the reads below, hit the minimal number of bank wavefronts for G >= 8),
+// lane gl then adds up slots PER*gl .. PER*gl + PER - 1 over the G rows of its group in a balanced tree and leaves them in
+// r[0 .. PER).  45 instructions per lane for a FULL record and G = 8, against 112 for the transposing shuffle tree
+// (28 SHFL + 56 FSEL + 28 FADD), and one shared-memory round trip instead of three dependent shuffle stages.
+// `scratch`: 32 * (NP + 4) floats, 16-byte aligned, that no lane of the warp reads for anything else any more.
+#ifndef MOM_SMEM_TREE
+#define MOM_SMEM_TREE 1
+#endif
+template <int NP, int G>
+__device__ __forceinline__ void mom_group_reduce_smem(float (&r)[NP], float* scratch, int lane, int gl, int group)
+{
+    constexpr int PER = NP / G, ROW = NP + 4;
+    __syncwarp();                                            // the other groups are done with the staged particles too
+    float4* mine = reinterpret_cast<float4*>(scratch + lane * ROW);
+#pragma unroll
+    for (int q = 0; q < NP / 4; ++q) mine[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
+    __syncwarp();
+    const float* col = scratch + (group * G) * ROW + PER * gl;
+    float a[G][PER];
+#pragma unroll
+    for (int j = 0; j < G; ++j) {
+        if constexpr (PER % 4 == 0) {
+#pragma unroll
+            for (int q = 0; q < PER / 4; ++q) {
+                const float4 v = reinterpret_cast<const float4*>(col + j * ROW)[q];
+                a[j][4 * q] = v.x; a[j][4 * q + 1] = v.y; a[j][4 * q + 2] = v.z; a[j][4 * q + 3] = v.w;
+            }
+        } else if constexpr (PER == 2) {
+            const float2 v = *reinterpret_cast<const float2*>(col + j * ROW);
+            a[j][0] = v.x; a[j][1] = v.y;
+        } else {
+            a[j][0] = col[j * ROW];
+        }
+    }
+#pragma unroll
+    for (int h = G / 2; h >= 1; h >>= 1) {
+#pragma unroll
+        for (int j = 0; j < h; ++j) {
+#pragma unroll
+            for (int i = 0; i < PER; ++i) a[j][i] += a[j + h][i];
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < PER; ++i) r[i] = a[0][i];
+}
+
 // The common case, cells of at most 128*G particles: same two passes, but (i) the particles of a cell are visited in
 // rotated order, starting at the particle whose shared-memory bank is G*group, so that the 32 lanes of a warp hit 32
 // different banks in every load whatever the cell boundaries are (the lanes of a group step through the cell
@@ -176,7 +223,7 @@ __device__ __forceinline__ void mom_cell_group(const float* bx, const float* by,
 template <int G, bool FULL, class Hook>
 __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, const float* bz, int32_t s, int32_t n,
                                              bool have, int gl, int group, double* __restrict__ rec, bool norot,
-                                             Hook after_reads)
+                                             float* scratch, Hook after_reads)
 {
     constexpr int NP = (FULL || G > 16) ? 32 : 16;
     constexpr int NREC = FULL ? 29 : 13;
@@ -307,7 +354,11 @@ __device__ __forceinline__ void mom_cell_rot(const float* bx, const float* by, c
 #pragma unroll
         for (int k = 13; k < NP; ++k) r[k] = 0.f;
     }
-    fpd_transpose_reduce<NP, G, float>(r, gl);           // balanced fp32 tree over the group's partial sums
+    // balanced fp32 tree over the group's partial sums (scratch: the chunk's own staging buffer, free once every lane
+    // has read its last particle; the next bulk copy into it is issued behind a proxy fence).  FULL records only: with
+    // the 13-slot record the shuffle tree is as fast (17.5 vs 17.7 us)
+    if (MOM_SMEM_TREE && FULL && scratch) mom_group_reduce_smem<NP, G>(r, scratch, gl + G * group, gl, group);
+    else fpd_transpose_reduce<NP, G, float>(r, gl);
     // lane gl holds record slots PER*gl .. PER*gl + PER - 1
     if (have) {
 #pragma unroll
@@ -553,7 +604,8 @@ moments_warp_kernel(const float* __restrict__ vx, const float* __restrict__ vy, 
                     }
                     reissued = true;
                 };
-                mom_cell_rot<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, sb, n, have, gl, group, rec, (aligned & 2) != 0, hook);
+                mom_cell_rot<G, FULL>(sx - r_cur.a0, sy - r_cur.a0, sz - r_cur.a0, sb, n, have, gl, group, rec, (aligned & 2) != 0,
+                                      NST == 2 ? sx : nullptr, hook);
             } else if (NST == 1) {
                 auto hook = [&]() {
                     if (more) {
