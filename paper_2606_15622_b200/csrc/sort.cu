@@ -231,7 +231,10 @@ scatter_kernel(int64_t np, const uint32_t* __restrict__ keys_in, const uint32_t*
 typedef fp_grid gather_grid;
 
 template <bool FROM_POS>
-__global__ void __launch_bounds__(256, 6)                   // 40 registers: all eight gathers of a trip in flight
+#ifndef GATHER_MINB
+#define GATHER_MINB 6
+#endif
+__global__ void __launch_bounds__(256, GATHER_MINB)         // 40 registers: all eight gathers of a trip in flight
 gather_kernel(int64_t np, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ skeys, int32_t ncell,
               int32_t* __restrict__ cell_start,
               const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ vx,

@@ -176,9 +176,14 @@ __device__ __forceinline__ void sw_hist(uint32_t* __restrict__ tile_hist, int nt
 // 37 vs 33 us at 4M particles.)
 // INFLOW: the grid has freestream faces (the re-insertion's call and registers stay out of the other instantiation).
 // (the reservoir variant is held to 64 registers -- four resident blocks: this kernel lives on loads in flight, 177 us at
-// 20M particles against 217 us with the 80 registers the re-insertion's call would otherwise take; the others to 40: six blocks)
+// 20M particles against 217 us with the 80 registers the re-insertion's call would otherwise take; the others to 32: eight
+// blocks, 33.1 -> 31.1 us in the step at 4M particles against six.  Loading the next trip's four values before working on
+// the current one is slower with six blocks (33.3 us) and with eight (35.1 us, spills).)
 template <bool WRITE_KEYS, bool INFLOW>
-__global__ void __launch_bounds__(256, INFLOW ? 4 : 6)
+#ifndef SW_MINB
+#define SW_MINB 8                      // 29 registers without a spill: eight resident blocks, 64 warps per SM
+#endif
+__global__ void __launch_bounds__(256, INFLOW ? 4 : SW_MINB)
 sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
           float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
           uint32_t* __restrict__ keys, uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask,
