@@ -12,7 +12,12 @@
 // triple.  Features, standardisation, fallback policy and under-relaxation are the same as in the fp32 kernel.
 #pragma once
 
-#define TC_WARPS 8
+#ifndef TC_WARPS
+#define TC_WARPS 9                               // 2 CTAs x 9 warps per SM = 2,664 tile slots: the 2,500 tiles of a 40k-cell grid
+#endif                                           // take ONE round (8 warps: 2,368 slots, a second round for 132 tiles: 30.2 vs 26.7 us)
+#ifndef TC_MINB
+#define TC_MINB 2
+#endif
 #define TC_THREADS (TC_WARPS * 32)
 #define TC_H 64                                  // hidden width
 // float4 fragments per layer: k-steps x n-tiles x 32 lanes
@@ -139,7 +144,7 @@ struct tc_params {
 // Persistent CTAs: the packed weights (80 KB) are copied to shared memory once per CTA, then every warp walks over
 // 16-cell tiles.  (One plain TF32 mma per product instead of the 3xTF32 triple was measured: 29.7 instead of 35.8 us
 // and 7e-3 of the output scale on the benchmark network -- outside north_star's 3e-3 for TF32, so it is not offered.)
-__global__ void __launch_bounds__(TC_THREADS, 2)
+__global__ void __launch_bounds__(TC_THREADS, TC_MINB)
 mlp_tc_kernel(const double* __restrict__ mom, const float* __restrict__ tau_cell, const float4* __restrict__ frags,
               const float* __restrict__ misc, float* __restrict__ coef, uint32_t* __restrict__ flags,
               const __grid_constant__ tc_params P)
