@@ -287,11 +287,7 @@ int fpi_closure_exact(fp_ctx* ctx, const double* mom_full, const float* tau_cell
     const int32_t ncell = ctx->ncell;
     const int blocks = fp_div_up(ncell, CE_TPB);
     const size_t smem = (size_t)CE_TPB * 90 * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
-        FP_CUDA_OK(ctx, cudaFuncSetAttribute(closure_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    static_assert((size_t)CE_TPB * 90 * sizeof(double) <= 48 * 1024, "above 48 KB the kernel needs cudaFuncAttributeMaxDynamicSharedMemorySize (per device)");
     fp_launch(closure_exact_kernel, blocks, CE_TPB, smem, stream, mom_full, tau_cell, ctx->p.tau, ctx->p.eps2_scale,
                                                                        ctx->p.min_count, ncell, coef, flags, kappa_est,
                                                                        with_update_constants ? ctx->cellc : nullptr, ctx->p.dt);
