@@ -18,7 +18,7 @@ static void fp_free_all(fp_ctx* c)
     cudaFree(c->key_a); cudaFree(c->key_b); cudaFree(c->idx_a); cudaFree(c->idx_b);
     cudaFree(c->block_hist); cudaFree(c->bin_total); cudaFree(c->cellc);
     if (c->h_err) cudaFreeHost(c->h_err);
-    cudaFree(c->d_errdev); cudaFree(c->d_tiebreak);
+    cudaFree(c->d_errdev); cudaFree(c->d_tiebreak); cudaFree(c->d_deferred);
     for (int s = 0; s < 2; ++s) { for (int k = 0; k < 5; ++k) cudaFree(c->hs_f[s][k]); cudaFree(c->hs_pid[s]); }
     cudaFree(c->hs_mom); cudaFree(c->hs_coef); cudaFree(c->hs_flags); cudaFree(c->hs_cell_start);
     if (c->hs_side) cudaStreamDestroy(c->hs_side);
@@ -84,6 +84,9 @@ extern "C" int fp_create(fp_ctx** out, const fp_params* h_params)
               cudaMalloc((void**)&c->d_errdev, 4) == cudaSuccess && cudaMemset(c->d_errdev, 0, 4) == cudaSuccess &&
               cudaMalloc((void**)&c->d_tiebreak, (1 + SW_TB_CAP) * sizeof(uint32_t)) == cudaSuccess &&
               cudaMemset(c->d_tiebreak, 0, (1 + SW_TB_CAP) * sizeof(uint32_t)) == cudaSuccess;
+    if (ok && c->p.wall[0].kind == FP_WALL_INFLOW)       // any freestream face implies wall[0] is one (checked above)
+        ok = cudaMalloc((void**)&c->d_deferred, ((size_t)c->p.max_particles + 1) * sizeof(uint32_t)) == cudaSuccess &&
+             cudaMemset(c->d_deferred, 0, sizeof(uint32_t)) == cudaSuccess;
     if (ok) *c->h_err = 0;
     if (!ok) { fp_free_all(c); delete c; cudaGetLastError(); return FP_ERR_CUDA; }
     *out = c;

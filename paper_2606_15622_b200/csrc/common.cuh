@@ -70,6 +70,8 @@ struct fp_ctx {
     uint32_t *h_err = nullptr, *d_err = nullptr;
     uint32_t *d_errdev = nullptr;    // device-memory copy of the word for kernels that must not run on bad boundaries
     uint32_t *d_tiebreak = nullptr;  // [1 + SW_TB_CAP]: count + particle indices whose reservoir accept/reject test was borderline in fp32
+    uint32_t *d_deferred = nullptr;  // [1 + max_particles], reservoir grids only: count + indices of the particles that left through a
+                                     // freestream face this step (re-inserted by sw_deferred_kernel)
     int       mom_occ[6] = {0, 0, 0, 0, 0, 0};       // resident CTAs per SM of moments_warp_kernel<2^k, *>
     int       mlp_tc_occ = 0, sw_occ[2] = {0, 0}, gather_occ = 0;
     bool      mlp_attr_w5 = false, mlp_attr_wd = false;

@@ -18,6 +18,7 @@ struct sw_params {
     fp_grid grid;                    // cell keys (slab-aware)
     float in_mu, in_sg, in_pen;     // freestream reservoir: mode of the flux density, sqrt(theta_inf), fl(U_inf,x * dt)
     uint32_t* tiebreak;              // [0] count, [1..] indices of re-inserted particles with a borderline fp32 accept/reject test
+    uint32_t* deferred;              // [0] count, [1..] indices of the particles that left through a freestream face (reservoir grids)
 };
 
 // One wall draw (R7): normal component sqrt(-2 theta_w ln u0) into the gas, tangentials
@@ -80,9 +81,12 @@ __device__ __noinline__ void sw_reinsert(const sw_params& P, uint32_t pid, uint3
 }
 
 // One particle: stream, walls, body, key.  pid is read only by particles that hit something.
-struct sw_moved { float x, y, v0, v1, v2; uint32_t key; bool redrawn; };
+struct sw_moved { float x, y, v0, v1, v2; uint32_t key; bool redrawn, deferred; };
 
-template <bool WRITE_KEYS, bool INFLOW>
+// INFLOW: 0 = the grid has no freestream face; 1 = a particle that leaves through one is re-inserted here (sw_reinsert);
+// 2 = it is only reported (deferred = true, nothing else of the result is valid): the streaming kernel lists it and
+// sw_deferred_kernel runs this function again on the untouched inputs with INFLOW = 1.
+template <bool WRITE_KEYS, int INFLOW>
 __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float yin, float v0, float v1,
                                             const uint32_t* __restrict__ pid, int64_t p)
 {
@@ -107,7 +111,10 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
                     xp = side ? __fsub_rn(xp, P.Lx) : __fadd_rn(xp, P.Lx);
                     if (xp < P.xmin) xp = P.xmin;
                     if (xp >= P.xmax) xp = P.xmax_in;
-                } else if (INFLOW && w.kind == FP_WALL_INFLOW) {
+                } else if (INFLOW == 2 && w.kind == FP_WALL_INFLOW) {
+                    sw_moved d; d.x = xin; d.y = yin; d.v0 = v0; d.v1 = v1; d.v2 = 0.0f; d.key = 0u; d.redrawn = false; d.deferred = true;
+                    return d;
+                } else if (INFLOW == 1 && w.kind == FP_WALL_INFLOW) {
                     sw_reinsert(P, pid[p], (uint32_t)p, P.ny > 1, xp, yp, v0, v1, v2);
                     redrawn = true; reinserted = true;
                 }
@@ -130,7 +137,10 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
                     yp = side ? __fsub_rn(yp, P.Ly) : __fadd_rn(yp, P.Ly);
                     if (yp < P.ymin) yp = P.ymin;
                     if (yp >= P.ymax) yp = P.ymax_in;
-                } else if (INFLOW && w.kind == FP_WALL_INFLOW) {
+                } else if (INFLOW == 2 && w.kind == FP_WALL_INFLOW) {
+                    sw_moved d; d.x = xin; d.y = yin; d.v0 = v0; d.v1 = v1; d.v2 = 0.0f; d.key = 0u; d.redrawn = false; d.deferred = true;
+                    return d;
+                } else if (INFLOW == 1 && w.kind == FP_WALL_INFLOW) {
                     sw_reinsert(P, pid[p], (uint32_t)p, true, xp, yp, v0, v1, v2);
                     redrawn = true;
                 }
@@ -154,7 +164,7 @@ __device__ __forceinline__ sw_moved sw_move(const sw_params& P, float xin, float
             }
         }
         sw_moved m;
-        m.x = xp; m.y = yp; m.v0 = v0; m.v1 = v1; m.v2 = v2; m.redrawn = redrawn; m.key = 0u;
+        m.x = xp; m.y = yp; m.v0 = v0; m.v1 = v1; m.v2 = v2; m.redrawn = redrawn; m.deferred = false; m.key = 0u;
         if (WRITE_KEYS) {
             m.key = (uint32_t)fpd_cell_key(xp, yp, P.grid);
         }
@@ -173,17 +183,17 @@ __device__ __forceinline__ void sw_hist(uint32_t* __restrict__ tile_hist, int nt
 }
 
 // One particle per thread, grid-stride.  (Four particles per thread with 128-bit accesses was measured slower:
-// 37 vs 33 us at 4M particles.)
-// INFLOW: the grid has freestream faces (the re-insertion's call and registers stay out of the other instantiation).
-// (the reservoir variant is held to 64 registers -- four resident blocks: this kernel lives on loads in flight, 177 us at
-// 20M particles against 217 us with the 80 registers the re-insertion's call would otherwise take; the others to 32: eight
-// blocks, 33.1 -> 31.1 us in the step at 4M particles against six.  Loading the next trip's four values before working on
-// the current one is slower with six blocks (33.3 us) and with eight (35.1 us, spills).)
-template <bool WRITE_KEYS, bool INFLOW>
+// 37 vs 33 us at 4M particles.)  29 registers without a spill: eight resident blocks, 64 warps per SM (33.1 -> 31.1 us in
+// the step at 4M particles against six; loading the next trip's four values before working on the current one is
+// slower with six blocks, 33.3 us, and with eight, 35.1 us, spills).
+// INFLOW: the grid has freestream faces.  A particle that leaves through one is not re-inserted here -- the call into
+// sw_reinsert would cost this kernel its registers (64 instead of 29: four resident blocks, 204 instead of ~165 us at
+// 20M particles) -- but put on a list; its arrays stay untouched and sw_deferred_kernel handles it.
 #ifndef SW_MINB
-#define SW_MINB 8                      // 29 registers without a spill: eight resident blocks, 64 warps per SM
+#define SW_MINB 8
 #endif
-__global__ void __launch_bounds__(256, INFLOW ? 4 : SW_MINB)
+template <bool WRITE_KEYS, bool INFLOW>
+__global__ void __launch_bounds__(256, SW_MINB)
 sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx,
           float* __restrict__ vy, float* __restrict__ vz, const uint32_t* __restrict__ pid,
           uint32_t* __restrict__ keys, uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask,
@@ -195,15 +205,42 @@ sw_kernel(int64_t np, float* __restrict__ x, float* __restrict__ y, float* __res
     // warp-uniform trip count: the histogram is a full-warp collective; a warp's 32 particles lie in one sort tile
     for (int64_t p0 = (int64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31); p0 < np; p0 += stride) {
         const int64_t p = p0 + lane;
-        const bool valid = p < np;
+        bool valid = p < np;
         uint32_t key = 0u;
         if (valid) {
-            const sw_moved m = sw_move<WRITE_KEYS, INFLOW>(P, x[p], y[p], vx[p], vy[p], pid, p);
-            x[p] = m.x; y[p] = m.y; key = m.key;
-            if (m.redrawn) { vx[p] = m.v0; vy[p] = m.v1; vz[p] = m.v2; }
-            if (WRITE_KEYS) keys[p] = key;
+            const sw_moved m = sw_move<WRITE_KEYS, INFLOW ? 2 : 0>(P, x[p], y[p], vx[p], vy[p], pid, p);
+            if (INFLOW && m.deferred) {
+                P.deferred[1u + atomicAdd(P.deferred, 1u)] = (uint32_t)p;     // at most once per particle: the list holds np entries
+                valid = false;                                                  // its histogram entry comes with its new position
+            } else {
+                x[p] = m.x; y[p] = m.y; key = m.key;
+                if (m.redrawn) { vx[p] = m.v0; vy[p] = m.v1; vz[p] = m.v2; }
+                if (WRITE_KEYS) keys[p] = key;
+            }
         }
         if (WRITE_KEYS && tile_hist) sw_hist(tile_hist, ntiles, p0 / SORT_TILE, valid, key, digit_mask, lane);
+    }
+}
+
+// The particles the streaming kernel listed (they left through a freestream face; ~1e-3 of the ensemble per step):
+// the whole move again from their untouched arrays, re-insertion included, then key and histogram entry.
+template <bool WRITE_KEYS>
+__global__ void __launch_bounds__(128)
+sw_deferred_kernel(float* __restrict__ x, float* __restrict__ y, float* __restrict__ vx, float* __restrict__ vy,
+                   float* __restrict__ vz, const uint32_t* __restrict__ pid, uint32_t* __restrict__ keys,
+                   uint32_t* __restrict__ tile_hist, int ntiles, uint32_t digit_mask, const __grid_constant__ sw_params P)
+{
+    fpd_pdl();
+    const uint32_t n = P.deferred[0];
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int64_t p = (int64_t)P.deferred[1u + i];
+        const sw_moved m = sw_move<WRITE_KEYS, 1>(P, x[p], y[p], vx[p], vy[p], pid, p);
+        x[p] = m.x; y[p] = m.y;
+        if (m.redrawn) { vx[p] = m.v0; vy[p] = m.v1; vz[p] = m.v2; }
+        if (WRITE_KEYS) {
+            keys[p] = m.key;
+            if (tile_hist) atomicAdd(&tile_hist[(size_t)(m.key & digit_mask) * ntiles + (size_t)(p / SORT_TILE)], 1u);
+        }
     }
 }
 
@@ -230,7 +267,7 @@ sw_tiebreak_kernel(float* __restrict__ vx, const uint32_t* __restrict__ pid, con
         vx[p] = (float)vn;
     }
     __syncthreads();
-    if (threadIdx.x == 0) P.tiebreak[0] = 0u;
+    if (threadIdx.x == 0) { P.tiebreak[0] = 0u; P.deferred[0] = 0u; }      // both lists are consumed: sw_deferred_kernel ran before
 }
 
 int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, float* vy, float* vz,
@@ -258,6 +295,7 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
         volatile float pen = q.wall[0].ux * q.dt; P.in_pen = pen;
     }
     P.tiebreak = ctx->d_tiebreak;
+    P.deferred = ctx->d_deferred;
     P.k0 = (uint32_t)q.seed; P.k1 = (uint32_t)(q.seed >> 32);
     P.step_lo = (uint32_t)step; P.step_hi = (uint32_t)(step >> 32);
     const int threads = 256;
@@ -285,9 +323,15 @@ int fpi_stream_walls(fp_ctx* ctx, int64_t np, float* x, float* y, float* vx, flo
         if (inflow) fp_launch(sw_kernel<false, true>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
         else        fp_launch(sw_kernel<false, false>, blocks, threads, 0, st, np, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
     }
-    if (inflow) fp_launch(sw_tiebreak_kernel, 1, 128, 0, st, vx, pid, P);
+    if (inflow) {
+        const int dblocks = 2 * ctx->num_sms;
+        if (keys_out) fp_launch(sw_deferred_kernel<true>, dblocks, 128, 0, st, x, y, vx, vy, vz, pid, keys_out,
+                                with_hist0 ? ctx->block_hist : nullptr, fp_div_up(np, SORT_TILE), (1u << fpi_sort_digit_bits(ctx)) - 1u, P);
+        else          fp_launch(sw_deferred_kernel<false>, dblocks, 128, 0, st, x, y, vx, vy, vz, pid, nullptr, nullptr, 0, 0u, P);
+        fp_launch(sw_tiebreak_kernel, 1, 128, 0, st, vx, pid, P);
+    }
     FP_LAUNCH_OK(ctx);
-    FP_COUNT(ctx, inflow ? 2 : 1);
+    FP_COUNT(ctx, inflow ? 3 : 1);
     return FP_OK;
 }
 
