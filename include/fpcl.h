@@ -11,7 +11,8 @@
  *  - Pointers are DEVICE pointers unless the name starts with h_ (host).  The caller owns every particle, grid,
  *    coefficient and weight buffer; the library never allocates or frees them.  The library owns only fp_ctx and
  *    its scratch.  Everything whose size follows from fp_params is allocated by fp_create (sort ping-pong buffers,
- *    digit histograms, per-cell update constants, the accumulators of the high-particles-per-cell paths).  Two
+ *    digit histograms, per-cell update constants, the accumulators of the high-particles-per-cell paths and, on grids
+ *    with a freestream face, a list of max_particles + 1 particle indices for the re-insertion pass).  Two
  *    pieces depend on later arguments and are allocated on FIRST USE unless fp_reserve was called: the packed
  *    parameters of a surrogate network (sized by its shape; a differently shaped network re-allocates) and the
  *    device staging buffers of fp_step_host.  A first-use allocation is a cudaMalloc and may stall the stream.
