@@ -93,6 +93,41 @@ def test_sort_two_array_path(gpu, wl, orc, monkeypatch):
     ctx.close()
 
 
+def test_sort_and_step_on_the_cylinder_grid(gpu, wl, orc):
+    """The cylinder case's 400 x 300 grid (17 key bits: 9 + 8 bit passes) in a context sized for more than 2^24
+    particles, a sparse ensemble with a dense corner (long runs of equal keys): the sort, then one whole fp_step whose
+    positions, ids and cell_start must match the oracle's stream + sort bit for bit (the stream kernel fills the first
+    pass's histogram).  (A 10-bit first digit, which would let the 19.9M-particle case travel packed, was built on this
+    test and dropped: its 1024-row tables cost the key passes 32 us more than the packed word saves.)"""
+    rng = np.random.default_rng(9)
+    nx, ny, n = 400, 300, 200_000
+    cfg = wl.make_config(nx, ny, 1.0, 1.0, 0.05, 1.0, wl.NO_WALLS, max_particles=(1 << 24) + 1)
+    st = dict(x=rng.uniform(0, nx, n).astype(np.float32), y=rng.uniform(0, ny, n).astype(np.float32),
+              vx=rng.normal(size=n).astype(np.float32), vy=rng.normal(size=n).astype(np.float32),
+              vz=rng.normal(size=n).astype(np.float32), pid=np.arange(n, dtype=np.uint32))
+    st["x"][::7] = rng.uniform(0, 40, st["x"][::7].shape[0]).astype(np.float32)        # a dense corner: long runs of equal keys
+    ref, ref_cs, ref_perm = orc.sort_by_cell(st, cfg)
+    ctx = gpu.Context(cfg)
+    out, cs, perm = ctx.sort_by_cell(gpu.to_device(st))
+    assert np.array_equal(cs.cpu().numpy(), ref_cs)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), ref_perm)
+    got = gpu.to_host(out)
+    for k in ("x", "y", "vx", "vy", "vz", "pid"):
+        assert np.array_equal(got[k].view(np.uint32), ref[k].view(np.uint32)), k
+    # fp_step: positions, ids and cell_start bit for bit against the oracle's stream + sort
+    import torch
+    a = gpu.to_device(st)
+    b = {k: torch.empty_like(v) for k, v in a.items()}
+    o = ctx.alloc_step_outputs(0)
+    ctx.step(a, b, 3, o, closure=0)
+    mid = orc.stream_walls(st, cfg, 3)
+    s2, cs2, _ = orc.sort_by_cell({k: np.ascontiguousarray(v) for k, v in mid.items()}, cfg)
+    assert np.array_equal(o["cell_start"].cpu().numpy(), cs2)
+    for k in ("x", "y", "pid"):
+        assert np.array_equal(b[k].cpu().numpy().view(np.uint32), np.ascontiguousarray(s2[k]).view(np.uint32)), k
+    ctx.close()
+
+
 def test_sort_three_passes(gpu, wl, orc):
     """More than 2^18 cells forces a third radix pass."""
     rng = np.random.default_rng(5)
