@@ -64,7 +64,7 @@ SEEDS = [1028, 1034, 1098, 1287,      # N = 2, cm 1: the energy rescaling is a s
          1076, 1077, 1136, 1204,      # N = 2 .. 6, cm 0: degenerate eps2 ~ 1/(tau theta), cubic term of ~3 thermal speeds
          1241, 5012,                  # 230 ppc with diffuse walls at Mach 13; reservoir faces on 1.2M particles (accept/reject flip)
          30172, 30773, 41721,         # bimodal Mach-9 cells of 2,000+ particles (range floor); at-rest tails in Mach-6 cells (fp64 sums)
-         40387, 41783,                # a 9-particle cell on the slice path; a two-particle cell whose energy scale is 0.3 of its terms
+         40387, 41783, 102080,        # a 9-particle cell on the slice path; two-particle cells whose energy scale is a small part of its terms
          1000, 1001, 1002, 1003]      # controls
 
 
