@@ -59,6 +59,7 @@ struct fp_ctx {
     uint32_t *key_a = nullptr, *key_b = nullptr, *idx_a = nullptr, *idx_b = nullptr;
     uint32_t *block_hist = nullptr;  // two tables [bins][nblocks]: even passes use the first, odd passes the second
     bool      sort_no_pack = false;  // FPCL_SORT_UNPACKED=1: always move (key, index) as two arrays (test hook)
+    bool      sort_slab_keys = false; // set by fp_slab_partition around its sort: the keys are destination slabs, not cell keys of the positions
     bool      hist0_clean = true;    // the first table is all zero (what the stream kernel's fused histogram needs)
     uint32_t *bin_total = nullptr;   // [bins]
     size_t    block_hist_elems = 0;

@@ -87,7 +87,7 @@ extern "C" int fp_slab_partition(fp_ctx* ctx, int64_t np,
     const int32_t ncell_saved = ctx->ncell, bits_saved = ctx->key_bits;
     int bits = 1;
     while ((1 << bits) < nslabs) ++bits;
-    ctx->ncell = nslabs; ctx->key_bits = bits;
+    ctx->ncell = nslabs; ctx->key_bits = bits; ctx->sort_slab_keys = true;
     int rc = FP_OK;
     if (np > 0) {
         const int nblocks = fp_div_up(np, SORT_TILE);
@@ -99,6 +99,6 @@ extern "C" int fp_slab_partition(fp_ctx* ctx, int64_t np,
     if (rc == FP_OK)
         rc = fpi_sort_with_keys(ctx, np, ctx->key_b, np > 0, x, y, vx, vy, vz, pid, x_out, y_out, vx_out, vy_out, vz_out, pid_out,
                                 slab_start, nullptr, st);
-    ctx->ncell = ncell_saved; ctx->key_bits = bits_saved;
+    ctx->ncell = ncell_saved; ctx->key_bits = bits_saved; ctx->sort_slab_keys = false;
     return rc;
 }

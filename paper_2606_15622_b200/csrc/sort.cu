@@ -103,7 +103,9 @@ __device__ __forceinline__ int dbits_of(int bins) { return 31 - __clz(bins); }
 // index bits + high-digit bits <= 32 the pair travels as one word between the passes: PACK_OUT (first pass) writes
 // (high digit << pack_bits) | index into keys_out, PACK_IN (second pass) reads that word, ranks by its digit and
 // writes only the index; the sorted keys are not stored (the gather recomputes them from the positions).
-enum { SORT_FIRST = 0, SORT_LATER = 1, SORT_PACK_OUT = 2, SORT_PACK_IN = 3 };
+// LATER_NOKEYS: the last pass of a two-array sort whose keys are cell keys: only the index is written, the gather recomputes
+// the keys from the positions (as after a packed sort).
+enum { SORT_FIRST = 0, SORT_LATER = 1, SORT_PACK_OUT = 2, SORT_PACK_IN = 3, SORT_LATER_NOKEYS = 4 };
 
 // The items of one tile: load, rank, scatter.  FULLT: every item of the tile exists (no bounds checks).
 template <int MODE, bool FULLT>
@@ -114,7 +116,7 @@ __device__ __forceinline__ void scatter_items(int64_t np, const uint32_t* __rest
                                               uint32_t (*cnt)[SORT_MAX_BINS], const uint32_t* bin_base)
 {
     constexpr bool FIRST_PASS = (MODE == SORT_FIRST || MODE == SORT_PACK_OUT);
-    constexpr bool HAS_IDX = (MODE == SORT_LATER);       // a separate index array comes in
+    constexpr bool HAS_IDX = (MODE == SORT_LATER || MODE == SORT_LATER_NOKEYS);       // a separate index array comes in
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t mask = (uint32_t)bins - 1u;
     const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_ITEMS) + lane;   // this lane's first item
@@ -162,6 +164,7 @@ __device__ __forceinline__ void scatter_items(int64_t np, const uint32_t* __rest
             const uint32_t dst = bin_base[d] + cnt[warp][d] + rank[i];
             if (MODE == SORT_PACK_OUT) keys_out[dst] = ((key[i] >> (shift + dbits_of(bins))) << pack_bits) | idx[i];
             else if (MODE == SORT_PACK_IN) idx_out[dst] = key[i] & ((1u << pack_bits) - 1u);
+            else if (MODE == SORT_LATER_NOKEYS) idx_out[dst] = idx[i];
             else { keys_out[dst] = key[i]; idx_out[dst] = idx[i]; }
             code = (((key[i] >> shift) >> dbits_of(bins)) & mask) << 20 | (dst / SORT_TILE);
         }
@@ -321,6 +324,8 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     int idx_bits = 1;
     while (idx_bits < 32 && ((int64_t)1 << idx_bits) < np) ++idx_bits;
     const bool packed = !ctx->sort_no_pack && passes == 2 && idx_bits + (bits - dbits) <= 32;
+    // two-array sorts of cell keys (20M particles: index + high digit do not fit one word) need not store the sorted keys either
+    const bool nokeys_last = !packed && passes >= 2 && !ctx->sort_slab_keys;
     const uint32_t* kin = keys;
     const uint32_t* iin = nullptr;
     uint32_t* kout = ctx->key_a;
@@ -341,6 +346,8 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
             fp_launch(scatter_kernel<SORT_PACK_IN>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, idx_bits, bins, idx_bits, next);
         else if (pass == 0)
             fp_launch(scatter_kernel<SORT_FIRST>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, 0, next);
+        else if (nokeys_last && pass + 1 == passes)
+            fp_launch(scatter_kernel<SORT_LATER_NOKEYS>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, 0, next);
         else
             fp_launch(scatter_kernel<SORT_LATER>, nblocks, SORT_THREADS, 0, st, np, kin, iin, kout, iout, table, ctx->bin_total, nblocks, shift, bins, 0, next);
         FP_LAUNCH_OK(ctx);
@@ -362,7 +369,7 @@ int fpi_sort_with_keys(fp_ctx* ctx, int64_t np, const uint32_t* keys, bool hist0
     const int gblocks = (int)(want < cap ? want : cap);
     const gather_grid Gd = fp_grid_of(ctx);
     if (ctx->ev_before_gather) FP_CUDA_OK(ctx, cudaStreamWaitEvent(st, ctx->ev_before_gather, 0));
-    if (packed)
+    if (packed || nokeys_last)
         fp_launch(gather_kernel<true>, gblocks, 256, 0, st, np, iin, kin, ncell, cell_start, x, y, vx, vy, vz, pid,
                   x_out, y_out, vx_out, vy_out, vz_out, pid_out, Gd);
     else
