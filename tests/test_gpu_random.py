@@ -6,6 +6,8 @@ tolerance -- two-particle cells whose energy rescaling cancels, hypersonic few-p
 rounding of the bulk velocity, re-emitted particles ten thermal speeds out in giant cells, a borderline accept/reject in the
 reservoir -- plus a few that always passed.  Every stage gets the ORACLE's output of the previous stage as its input, so the
 strict tolerances of tests/parity_util.py apply (1e-6 moments and velocities, 1e-5 coefficients, integers bit for bit)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -66,6 +68,11 @@ SEEDS = [1028, 1034, 1098, 1287,      # N = 2, cm 1: the energy rescaling is a s
          30172, 30773, 41721,         # bimodal Mach-9 cells of 2,000+ particles (range floor); at-rest tails in Mach-6 cells (fp64 sums)
          40387, 41783, 102080,        # a 9-particle cell on the slice path; two-particle cells whose energy scale is a small part of its terms
          1000, 1001, 1002, 1003]      # controls
+
+
+# FPCL_RANDOM_CASES=N adds N fresh seeds (the sweep this file's seeds were found with; ~20 cases per second).  11,000 such
+# cases left one miss on the final build: 1.03x in a two-particle cell at Mach 52.
+SEEDS += list(range(500000, 500000 + int(os.environ.get("FPCL_RANDOM_CASES", "0"))))
 
 
 @pytest.mark.parametrize("seed", SEEDS)
